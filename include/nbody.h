@@ -1,0 +1,176 @@
+/*
+ * include/nbody.h -- C ABI of libnbody.so: the B200 (sm_100a) hot path of the block-time-step Hermite direct
+ * N-body method benchmarked in arXiv:1312.1789.
+ *
+ * Method statement.  The paper names the scheme only -- "individual hierarchically block time-steps with the
+ * high (4th, 6th and 8th) order Hermite integration schemes" (abstract), forces on the GPU
+ * (section 2), "mixed (fp32 + fp64) precision" (Fig. 1 caption) -- and prints no
+ * formula.  The operations below are therefore defined by DESIGN.md section 3 (readings R1..R12, restating
+ * SURVEY.md 8(c) items c-1..c-14), each cited per call.
+ *
+ * Conventions (all calls)
+ *   - G = 1, potential negative, one Plummer softening eps2 for all pairs (R3, R11).
+ *   - `order` p is 4, 6 or 8; K = p/2 force derivatives (acc, jerk | +snap | +crackle).
+ *   - Unless a parameter is marked HOST, every array pointer is a DEVICE pointer into caller-owned memory,
+ *     fp64, contiguous; 3-vectors are row-major [n][3].  `stream` is a cudaStream_t passed as void* (NULL =
+ *     the legacy default stream).  Device-pointer calls only enqueue work and return; they never synchronise.
+ *   - The ctx owns scratch only (packed j-store, split partials, staging for the *_host calls).  It never frees
+ *     or keeps caller memory.  A ctx is bound to the device given at creation and is not thread-safe.
+ *   - Every call returns an int status: NBODY_OK (0) or a negative NBODY_E* code; nothing aborts, throws or
+ *     prints.  nbody_strerror() maps a code to a static string.
+ *   - There is no CPU fallback anywhere: without a CUDA device nbody_create() returns NBODY_ECUDA.
+ */
+#ifndef NBODY_H_
+#define NBODY_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NBODY_OK       0
+#define NBODY_EINVAL  (-1) /* bad argument: order, sizes, NULL where required, eps2 < 0, misalignment          */
+#define NBODY_ESTATE  (-2) /* call order: force before predict, force order > order of the last predict       */
+#define NBODY_ECUDA   (-3) /* a CUDA runtime call or launch failed; see nbody_last_cuda_error()               */
+#define NBODY_ENOMEM  (-4) /* device or host allocation failed                                                */
+
+typedef struct nbody_ctx nbody_ctx;
+
+/* ABI version of this header (bumped on any signature change). */
+int nbody_abi_version(void);
+
+/* Static description of `code`; never NULL. */
+const char *nbody_strerror(int code);
+
+/* Create a context for up to n_capacity particles on CUDA device `device`.  Allocates the packed j-store
+ * (4 planes x 16 B x n_capacity rounded up to the j-tile), the split-partial scratch and small control
+ * blocks with cudaMalloc.  *out is set only on success.  Synchronises the device. */
+int nbody_create(nbody_ctx **out, int64_t n_capacity, int device);
+
+/* Free everything the ctx owns (synchronises the device first).  NULL is a no-op. */
+int nbody_destroy(nbody_ctx *ctx);
+
+/* The cudaError_t (as int) of the last failing CUDA call made through this ctx, 0 if none. */
+int nbody_last_cuda_error(const nbody_ctx *ctx);
+
+/* Tuning / evidence knobs (host-side integers; unknown key -> NBODY_EINVAL).
+ *   "diff_mode"   0 = literal: d = fl32(x_j - x_i), subtraction in fp64 (DADD + F2F)          [default]
+ *                 1 = double-single: x = hi + lo (two fp32), d = (hi_j - hi_i) + (lo_j - lo_i)  (R10 note)
+ *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
+ *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 4, 16, 64, 256)
+ */
+int nbody_set_option(nbody_ctx *ctx, const char *key, int64_t value);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_predict -- a-2, Taylor predictor of ALL n particles to the block time t_now (R5 = SURVEY c-5;
+ * PAPER.md:43 "Hermite integration scheme" implies predict-evaluate-correct).
+ *   tau = t_now - t[i];  D_k = a_derivs[k] = a^(k)(t_i), k = 0 .. order-3 (entries above that are ignored and
+ *   may be NULL):
+ *     x_p = x + v tau + Sum_k D_k tau^(k+2)/(k+2)!      v_p = v + Sum_k D_k tau^(k+1)/(k+1)!
+ *     a_p = Sum_k D_k tau^k/k!  (order >= 6)            j_p = Sum_{k>=1} D_k tau^(k-1)/(k-1)!  (order == 8)
+ *   evaluated in fp64 by Horner, innermost term first, with c_k = tau / k, no FMA contraction (bit-exact
+ *   against the oracle, R12).  Results go to the ctx-owned packed j-store: x_p as fp64, v_p a_p j_p m rounded
+ *   to fp32 (round-to-nearest-even).  The j-store stays valid until the next nbody_predict on this ctx.
+ *   a_derivs is a HOST array of 6 device pointers; it is read during the call only.
+ * Errors: EINVAL (order, n < 0, n > capacity, NULL t/m/x/v or NULL a_derivs[k] for k <= order-3).
+ * n == 0 is a successful no-op that marks the j-store as holding 0 particles.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_predict(nbody_ctx *ctx, int64_t n, double t_now, int order,
+                  const double *t, const double *m, const double *x, const double *v,
+                  const double *const a_derivs[6] /* HOST array of device pointers */, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_force -- a-3 (+ a-3b), the O(n_act * n) hot loop (R1..R4, R10 = SURVEY c-1..c-4, c-12; PAPER.md:43,
+ * PAPER.md:65 eq. (1) alpha-term; mixed precision PAPER.md:31).
+ *   For each active i (index into the j-store of the last nbody_predict), over all j != i (excluded BY INDEX):
+ *     r = x_j - x_i (fp64 subtraction, rounded to fp32), v = v_j - v_i, a = a_j - a_i, jk = j_j - j_i (fp32)
+ *     s2 = r.r + eps2;  q = m_j / s2^(3/2);  alpha = (r.v)/s2;  beta = (v.v + r.a)/s2 + alpha^2
+ *     gamma = (3 v.a + r.jk)/s2 + alpha (3 beta - 4 alpha^2)
+ *     A = q r;  J = q v - 3 alpha A;  S = q a - 6 alpha J - 3 beta A;  C = q jk - 9 alpha S - 9 beta J - 3 gamma A
+ *     acc = Sum A, jerk = Sum J, snap = Sum S (order >= 6), crackle = Sum C (order == 8), pot = -Sum m_j/sqrt(s2)
+ *   fp32 pair arithmetic (MUFU rsqrt), per-thread fp32 partial sums over <= 64 consecutive j, then fp64.
+ *   Outputs are in ACTIVE-LIST order: acc, jerk, snap, crackle [n_act][3], pot [n_act], fully overwritten.
+ *   snap may be NULL when order < 6, crackle when order < 8 (they are not written then).
+ *   active_idx: device int32 [n_act], each in [0, n), unique (ascending recommended, not required).
+ *   Deterministic: the same inputs and options give bit-identical outputs run to run.
+ * Errors: EINVAL (order, n_act < 0, n_act > n, eps2 < 0 or NaN, NULL required pointer), ESTATE (no predict yet,
+ * or order > the order of the last predict).  n_act == 0 is a successful no-op.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_force(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order, double eps2,
+                double *acc, double *jerk, double *snap, double *crackle, double *pot, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_correct -- a-4, Hermite corrector + Aarseth-style block time step with power-of-two quantisation for the
+ * active particles (R6..R9 = SURVEY c-6..c-9; "hierarchically block time-steps").
+ *   For each active i, h = dt[i], 0 = stored state at t[i], 1 = force-call values at t_now:
+ *     compact two-point Hermite corrector for v then x (R6), interpolated a^(K..2K-1)(t_now) (R7),
+ *     dt_crit = eta (A^(1)/A^(p-2))^(1/(p-3)), A^(k) = sqrt(|a^(k-1)||a^(k+1)| + |a^(k)|^2) (R8),
+ *     dt_new = 2^floor(log2 dt_crit) by exact comparisons; <= 2 dt_old; doubling only if t_now is a multiple
+ *     of the doubled step; clamped to [dt_min, dt_max] (R9).
+ *   In place: x, v, a_derivs[0..order-1], pot_state, t := t_now, dt := dt_new for the active rows.
+ *   fp64, no FMA contraction, IEEE div/sqrt, operation order as DESIGN.md section 3 states: bit-exact vs oracle.
+ *   acc .. pot are the force-call outputs in active-list order.  a_derivs is a HOST array of 8 device pointers,
+ *   entries 0 .. order-1 required.  dt_min, dt_max must be exact powers of two.
+ * Errors: EINVAL (order, n_act < 0, NULL required pointer, eta <= 0, dt_min/dt_max not powers of two or
+ * dt_min > dt_max).  n_act == 0 is a successful no-op.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_correct(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order,
+                  double t_now, double eta, double dt_min, double dt_max,
+                  double *t, double *dt, double *x, double *v,
+                  double *const a_derivs[8] /* HOST array of device pointers */, double *pot_state,
+                  const double *acc, const double *jerk, const double *snap, const double *crackle,
+                  const double *pot, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_initial_dt -- start-up step of the bootstrap (R9b = SURVEY c-10): dt_i = 2^floor(log2(eta_s |a|/|j|))
+ * clamped to [dt_min, dt_max]; |j| == 0 -> dt_max.  acc, jerk, dt: device [n][3], [n][3], [n].  Bit-exact.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double *jerk,
+                     double eta_s, double dt_min, double dt_max, double *dt, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_next_block -- a-1, block selection on the device (R9c = SURVEY c-11): t_next = min_i (t[i] + dt[i])
+ * (exact for dyadic values); active = { i : t[i] + dt[i] == t_next } ascending.  Writes active_idx (device
+ * int32, capacity n) and returns t_next and n_act through HOST pointers; this call synchronises `stream`.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
+                     int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);
+
+/* Test hook: export the packed j-store of the last predict (n particles) into plain arrays.  xp fp64 [n][3];
+ * vp, ap, jp fp32 [n][3] (ap/jp may be NULL; ap requires order >= 6, jp order == 8 else EINVAL); m32 fp32 [n]. */
+int nbody_get_predicted(nbody_ctx *ctx, double *xp, float *vp, float *ap, float *jp, float *m32, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_force_host -- the same path (predict at t_now, then force) with HOST buffers: every pointer below is a
+ * HOST pointer (pageable or pinned).  Copies t, m, x, v, D_0..D_{order-3} and active_idx to ctx-owned device
+ * staging, runs nbody_predict + nbody_force, copies acc/jerk/snap/crackle/pot back, and returns after the
+ * results are in host memory (synchronises).  Used for the end-to-end measurement; results are identical to
+ * the device-pointer calls.  h2d_bytes / d2h_bytes (may be NULL) receive the bytes copied each way.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_force_host(nbody_ctx *ctx, int64_t n, double t_now, int order,
+                     const double *t, const double *m, const double *x, const double *v,
+                     const double *const a_derivs[6] /* HOST array of HOST pointers */,
+                     const int32_t *active_idx, int64_t n_act, double eps2,
+                     double *acc, double *jerk, double *snap, double *crackle, double *pot,
+                     int64_t *h2d_bytes, int64_t *d2h_bytes);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_probe_peak -- chip micro-probes used for the roofline denominators.  Runs a
+ * register-only loop of one instruction class on every SM for about `millis` ms and returns the achieved
+ * rate in 1e12 thread-operations per second through *tera_ops_host (an FFMA counts as ONE operation).
+ *   kind 0 = FFMA (fp32), 1 = DADD (fp64 add), 2 = F2F fp64->fp32 convert, 3 = MUFU.RSQ, 4 = DADD+F2F pair.
+ * Synchronises.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_probe_peak(nbody_ctx *ctx, int kind, int millis, double *tera_ops_host);
+
+/* Kernel launches issued through this ctx since creation (all kernels of this library). */
+int64_t nbody_launch_count(const nbody_ctx *ctx);
+
+/* Geometry of the last nbody_force call (for tests / bench): lanes, j-splits, CTAs of the force kernel. */
+int nbody_last_force_geometry(const nbody_ctx *ctx, int *i_per_thread, int *j_lanes, int *j_splits, int64_t *ctas);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBODY_H_ */

@@ -1,0 +1,82 @@
+// libnbody.so, translation unit 3: register-only micro-probes of the instruction classes K_force is made of.
+// They give the "measured" denominators beside the nominal FP32 peak: thread-operations
+// per second of FFMA, DADD, F2F (fp64 -> fp32), MUFU.RSQ, and the DADD+F2F pair, each on every SM at once.
+#include "nbody_internal.h"
+
+namespace nbody {
+namespace {
+
+constexpr int kProbeIters = 4096;
+constexpr int kProbeChains = 8;
+
+template <int KIND>
+__global__ void __launch_bounds__(256) k_probe(float *sink, float seed) {
+    float f[kProbeChains];
+    double d[kProbeChains];
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) {
+        f[c] = seed + (float)(threadIdx.x + c);
+        d[c] = (double)seed + (double)(threadIdx.x * 3 + c);
+    }
+    const float b = 0.999f + seed, cc = 1e-3f;
+    const double db = 1e-3 + (double)seed;
+#pragma unroll 1
+    for (int it = 0; it < kProbeIters; ++it) {
+#pragma unroll
+        for (int c = 0; c < kProbeChains; ++c) {
+            if (KIND == 0) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[c]) : "f"(b), "f"(cc));
+            if (KIND == 1) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(d[c]) : "d"(db));
+            if (KIND == 2) asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(f[c]) : "d"(d[c]));
+            if (KIND == 3) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f[c]));
+            if (KIND == 4) {
+                double t;
+                asm volatile("add.rn.f64 %0, %1, %2;" : "=d"(t) : "d"(d[c]), "d"(db));
+                asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(f[c]) : "d"(t));
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) s += f[c] + (float)d[c];
+    if (s == 123.456f) sink[0] = s;  // never true in practice; keeps the chains live
+}
+
+typedef void (*probe_fn)(float *, float);
+const probe_fn kProbes[5] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>};
+
+}  // namespace
+
+int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
+    NB_CUDA(c, cudaSetDevice(c->device));
+    float *sink = nullptr;
+    NB_CUDA(c, cudaMalloc(&sink, sizeof(float)));
+    cudaEvent_t e0, e1;
+    NB_CUDA(c, cudaEventCreate(&e0));
+    NB_CUDA(c, cudaEventCreate(&e1));
+    const int grid = c->sm_count * 8;  // 2048 threads per SM
+    const double ops_per_launch = (double)grid * 256.0 * kProbeIters * kProbeChains * (kind == 4 ? 2.0 : 1.0);
+    double best = 0.0, spent = 0.0;
+    int rc = NBODY_OK;
+    for (int rep = 0; rep < 100000 && spent < (double)millis; ++rep) {
+        cudaEventRecord(e0, 0);
+        kProbes[kind]<<<grid, 256>>>(sink, 0.0f);
+        c->launches += 1;
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        spent += ms;
+        if (rep > 0 && ms > 0.f) {
+            const double rate = ops_per_launch / (ms * 1e-3) / 1e12;
+            if (rate > best) best = rate;
+        }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    *tera_ops = best;
+    return rc;
+}
+
+}  // namespace nbody
