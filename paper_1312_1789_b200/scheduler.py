@@ -1,0 +1,104 @@
+"""Thin host block scheduler ("individual hierarchically block time-steps").
+
+Holds the fp64 SoA state as torch CUDA tensors (device memory only -- no torch arithmetic on the path) and drives
+the C-ABI calls per block:  next_block -> predict -> force -> correct.  Bootstrap = DESIGN.md R9b (SURVEY c-10).
+"""
+import numpy as np
+import torch
+
+from . import nbody
+
+
+class Integrator:
+    def __init__(self, m, x, v, order, eps2, eta=0.1, eta_s=0.01, dt_min=2.0**-30, dt_max=2.0**-4, device=0,
+                 ctx=None):
+        assert order in (4, 6, 8)
+        self.order, self.eps2, self.eta, self.eta_s = order, float(eps2), float(eta), float(eta_s)
+        self.dt_min, self.dt_max = float(dt_min), float(dt_max)
+        self.dev = torch.device("cuda", device)
+        n = int(np.asarray(m).shape[0])
+        self.n = n
+        self.ctx = ctx if ctx is not None else nbody.Context(n, device)
+        up = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.dev)
+        self.m, self.x, self.v = up(m), up(x), up(v)
+        z = lambda *s: torch.zeros(*s, dtype=torch.float64, device=self.dev)
+        self.D = [z(n, 3) for _ in range(8)]
+        self.pot = z(n)
+        self.t = z(n)
+        self.dt = z(n)
+        # force outputs (active-list order) and the active list
+        self.acc, self.jerk, self.snap, self.crk = z(n, 3), z(n, 3), z(n, 3), z(n, 3)
+        self.fpot = z(n)
+        self.active = torch.zeros(n, dtype=torch.int32, device=self.dev)
+        self.all_idx = torch.arange(n, dtype=torch.int32, device=self.dev)
+        self.time = 0.0
+        self.blocks = 0
+        self.pairs = 0
+
+    # ---- R9b bootstrap: order-4 force at tau = 0, then (p >= 6) an order-8 force with those a, j ----
+    def bootstrap(self, fixed_dt=None):
+        c, n = self.ctx, self.n
+        c.predict(n, 0.0, 4, self.t, self.m, self.x, self.v, self.D)
+        c.force(self.all_idx, n, 4, self.eps2, self.acc, self.jerk, None, None, self.fpot)
+        self.D[0].copy_(self.acc)
+        self.D[1].copy_(self.jerk)
+        self.pot.copy_(self.fpot)
+        if self.order >= 6:
+            # order-8 predictor at tau = 0 with D = (a, j, 0, 0, 0, 0) puts a, j into the j-store
+            c.predict(n, 0.0, 8, self.t, self.m, self.x, self.v, self.D)
+            c.force(self.all_idx, n, 8, self.eps2, self.acc, self.jerk, self.snap, self.crk, self.fpot)
+            self.D[2].copy_(self.snap)
+            self.D[3].copy_(self.crk)
+        if fixed_dt is not None:
+            self.dt.fill_(float(fixed_dt))
+        else:
+            c.initial_dt(n, self.D[0], self.D[1], self.eta_s, self.dt_min, self.dt_max, self.dt)
+
+    def block_step(self):
+        c, n, p = self.ctx, self.n, self.order
+        t_next, n_act = c.next_block(n, self.t, self.dt, self.active)
+        c.predict(n, t_next, p, self.t, self.m, self.x, self.v, self.D)
+        c.force(self.active, n_act, p, self.eps2, self.acc, self.jerk, self.snap if p >= 6 else None,
+                self.crk if p >= 8 else None, self.fpot)
+        c.correct(self.active, n_act, p, t_next, self.eta, self.dt_min, self.dt_max, self.t, self.dt, self.x, self.v,
+                  self.D, self.pot, self.acc, self.jerk, self.snap if p >= 6 else None,
+                  self.crk if p >= 8 else None, self.fpot)
+        self.time = t_next
+        self.blocks += 1
+        self.pairs += n_act * n
+        return t_next, n_act
+
+    def integrate(self, t_end, max_blocks=10**9):
+        """Advance until the next block time would exceed t_end."""
+        hist = {}
+        while self.blocks < max_blocks:
+            # peek: the selection itself tells us t_next; stop when it passes t_end
+            t_next, n_act = self.ctx.next_block(self.n, self.t, self.dt, self.active)
+            if t_next > t_end:
+                break
+            p = self.order
+            c = self.ctx
+            c.predict(self.n, t_next, p, self.t, self.m, self.x, self.v, self.D)
+            c.force(self.active, n_act, p, self.eps2, self.acc, self.jerk, self.snap if p >= 6 else None,
+                    self.crk if p >= 8 else None, self.fpot)
+            c.correct(self.active, n_act, p, t_next, self.eta, self.dt_min, self.dt_max, self.t, self.dt, self.x,
+                      self.v, self.D, self.pot, self.acc, self.jerk, self.snap if p >= 6 else None,
+                      self.crk if p >= 8 else None, self.fpot)
+            self.time = t_next
+            self.blocks += 1
+            self.pairs += n_act * self.n
+            b = int(n_act).bit_length() - 1
+            hist[b] = hist.get(b, 0) + 1
+        return hist
+
+    def energy(self):
+        """E = Sum 1/2 m v^2 + 1/2 Sum m pot with pot from a synchronised order-4 all-active call (c-11).  The
+        two dot products are diagnostics taken on the host in fp64."""
+        assert bool((self.t == self.t[0]).all())
+        t0 = float(self.t[0])
+        self.ctx.predict(self.n, t0, 4, self.t, self.m, self.x, self.v, self.D)
+        self.ctx.force(self.all_idx, self.n, 4, self.eps2, self.acc, self.jerk, None, None, self.fpot)
+        m = self.m.cpu().numpy()
+        v = self.v.cpu().numpy()
+        pot = self.fpot.cpu().numpy()
+        return float(0.5 * np.sum(m * np.sum(v * v, axis=1)) + 0.5 * np.sum(m * pot))

@@ -1,0 +1,219 @@
+"""-m gpu tests of corrector / time step / block selection (bit-exact vs the oracle), the host scheduler
+(end-to-end block-step integration vs the oracle's own driver), error codes and the host-buffer path."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_1312_1789_b200 import workloads as W
+from tests import gpu_util as U
+
+
+@pytest.fixture(scope="module")
+def nb():
+    from paper_1312_1789_b200 import nbody
+    return nbody
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    return oracle
+
+
+def _state(config, n, order, seed_stream=11):
+    """A mid-run looking state: positions/velocities of the cluster, D_k from the oracle bootstrap, per-particle
+    dyadic t, dt with every particle of the active list due at t_now."""
+    c = W.cluster(config, n)
+    D = U.oracle_bootstrap_derivs(c, 8)
+    t, dt = W.predictor_times(c["x"])
+    return c, D, t, dt
+
+
+@pytest.mark.parametrize("order", [4, 6, 8])
+def test_correct_bit_exact(nb, O, order):
+    import torch
+    n = 3001
+    c, D, t, dt = _state(3, n, order)
+    t_now = 2.0**-10
+    rng = W.rng_for(3, 21)
+    idx = W.active_list(n, 1203, rng)
+    # force inputs at t1: the oracle's force on the oracle's prediction (any fp64 arrays would do: the corrector
+    # is compared on identical inputs)
+    xp, vp, ap, jp = O.predict(t_now, order, t, c["x"], c["v"], D)
+    acc, jerk, snap, crk, pot = O.force(c["m"], xp, vp, ap, jp, idx, order, c["eps2"])
+    for eta in (0.1, 0.02, 0.75):
+        # oracle
+        ot, odt, ox, ov = t.copy(), dt.copy(), c["x"].copy(), c["v"].copy()
+        oD = [d.copy() for d in D]
+        opot = np.zeros(n)
+        O.correct(idx, order, t_now, eta, 2.0**-30, 2.0**-4, ot, odt, ox, ov, oD, opot, acc, jerk, snap, crk, pot)
+        # GPU
+        gt, gdt, gx, gv = U.dev(t), U.dev(dt), U.dev(c["x"]), U.dev(c["v"])
+        gD = [U.dev(d) for d in D]
+        gpot = U.zeros(n)
+        ctx = nb.Context(n)
+        ctx.correct(U.dev(idx), idx.shape[0], order, t_now, eta, 2.0**-30, 2.0**-4, gt, gdt, gx, gv, gD, gpot,
+                    U.dev(acc), U.dev(jerk), None if snap is None else U.dev(snap),
+                    None if crk is None else U.dev(crk), U.dev(pot))
+        torch.cuda.synchronize()
+        assert np.array_equal(gt.cpu().numpy(), ot)
+        assert np.array_equal(gdt.cpu().numpy(), odt), "block time steps differ"
+        assert np.array_equal(gx.cpu().numpy(), ox)
+        assert np.array_equal(gv.cpu().numpy(), ov)
+        assert np.array_equal(gpot.cpu().numpy(), opot)
+        for k in range(order):
+            assert np.array_equal(gD[k].cpu().numpy(), oD[k]), "a^(%d) differs" % k
+        for k in range(order, 8):
+            assert np.array_equal(gD[k].cpu().numpy(), D[k])  # untouched
+        assert len(np.unique(odt[idx])) > 1  # the test exercises several step levels
+        ctx.close()
+
+
+def test_initial_dt_and_next_block_bit_exact(nb, O):
+    import torch
+    n = 70001  # several selection chunks (2048 per CTA) and a ragged tail
+    c = W.cluster(2, n)
+    idx = np.arange(n, dtype=np.int32)
+    rng = W.rng_for(2, 5)
+    acc = rng.normal(size=(n, 3)) * np.exp(rng.uniform(-3, 3, (n, 1)))
+    jerk = rng.normal(size=(n, 3)) * np.exp(rng.uniform(-3, 8, (n, 1)))
+    jerk[17] = 0.0
+    ref = O.initial_dt(acc, jerk, 0.01, 2.0**-30, 2.0**-4)
+    ctx = nb.Context(n)
+    gdt = U.zeros(n)
+    ctx.initial_dt(n, U.dev(acc), U.dev(jerk), 0.01, 2.0**-30, 2.0**-4, gdt)
+    torch.cuda.synchronize()
+    assert np.array_equal(gdt.cpu().numpy(), ref)
+    assert ref[17] == 2.0**-4
+    # block selection at several stages of a synthetic schedule
+    t = np.zeros(n)
+    dt = ref.copy()
+    act = torch.zeros(n, dtype=torch.int32, device="cuda")
+    for step in range(6):
+        tn, oidx = O.next_block(t, dt)
+        gtn, gna = ctx.next_block(n, U.dev(t), U.dev(dt), act)
+        assert gtn == tn and gna == oidx.shape[0]
+        assert np.array_equal(act[:gna].cpu().numpy(), oidx)
+        t[oidx] = tn  # advance the block (keep dt): next selection differs
+        if step == 3:
+            dt[oidx] *= 0.5
+    # all due at once
+    t[:] = 0.25
+    dt[:] = 0.125
+    gtn, gna = ctx.next_block(n, U.dev(t), U.dev(dt), act)
+    assert gtn == 0.375 and gna == n and np.array_equal(act.cpu().numpy(), idx)
+    ctx.close()
+
+
+@pytest.mark.parametrize("order", [4, 6, 8])
+def test_block_integration_vs_oracle(nb, O, order):
+    """Scheduler end to end on a small cluster with a central BH: same block sequence (bit-exact membership while
+    the trajectories agree) and x, v close to the oracle's own integration after a few dozen blocks."""
+    import torch
+    from oracle import integrate as OI
+    from paper_1312_1789_b200.scheduler import Integrator
+    c = W.cluster(5, 513)
+    eps2 = 1e-6
+    so = OI.bootstrap(c["m"], c["x"], c["v"], order, eps2)
+    g = Integrator(c["m"], c["x"], c["v"], order, eps2)
+    g.bootstrap()
+    torch.cuda.synchronize()
+    # bootstrap forces within tolerance; the first time steps may differ only where dt_crit sits on a power of two
+    assert U.rel_vec(g.D[0].cpu().numpy(), so.D[0]) < 1e-5
+    assert U.rel_vec(g.D[1].cpu().numpy(), so.D[1]) < 1e-4
+    same = np.mean(g.dt.cpu().numpy() == so.dt)
+    assert same > 0.98
+    # run both from the ORACLE's bootstrap state so that block membership can be compared bit for bit
+    for k in range(8):
+        g.D[k].copy_(U.dev(so.D[k]))
+    g.dt.copy_(U.dev(so.dt))
+    g.pot.copy_(U.dev(so.pot))
+    nblk = 40
+    for b in range(nblk):
+        tn_o, idx_o = OI.block_step(so, eps2, 0.1, 2.0**-30, 2.0**-4)
+        tn_g, na_g = g.block_step()
+        assert tn_g == tn_o and na_g == idx_o.shape[0], "block %d differs" % b
+        assert np.array_equal(g.active[:na_g].cpu().numpy(), idx_o)
+    torch.cuda.synchronize()
+    assert np.array_equal(g.t.cpu().numpy(), so.t)
+    assert np.max(np.abs(g.x.cpu().numpy() - so.x)) < 1e-9
+    assert np.max(np.abs(g.v.cpu().numpy() - so.v)) < 1e-7
+    # time steps are a decision taken from slightly different (mixed-precision) forces: nearly all identical
+    assert np.mean(g.dt.cpu().numpy() == so.dt) > 0.97
+
+
+def test_energy_conservation_gpu(nb):
+    """Short 6th-order block integration of a 1024-body Plummer sphere: |dE/E| small (invariant, no oracle)."""
+    from paper_1312_1789_b200.scheduler import Integrator
+    c = W.cluster(1)
+    g = Integrator(c["m"], c["x"], c["v"], 6, 1e-4, dt_max=2.0**-5)
+    g.bootstrap()
+    e0 = g.energy()
+    g.integrate(2.0**-3)
+    assert g.time == 2.0**-3 and bool((g.t == 2.0**-3).all())
+    e1 = g.energy()
+    assert abs(e0 + 0.25) < 0.03
+    assert abs((e1 - e0) / e0) < 1e-6
+
+
+def test_error_codes(nb):
+    import torch
+    ctx = nb.Context(100)
+    z = U.zeros(100, 3)
+    z1 = U.zeros(100)
+    idx = torch.arange(100, dtype=torch.int32, device="cuda")
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.force(idx, 10, 4, 1e-4, z, z, None, None, z1)
+    assert e.value.code == nb.ESTATE  # force before predict
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.predict(101, 0.0, 4, z1, z1, z, z, [z, z])
+    assert e.value.code == nb.EINVAL  # n > capacity
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.predict(100, 0.0, 5, z1, z1, z, z, [z, z])
+    assert e.value.code == nb.EINVAL  # order
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.predict(100, 0.0, 6, z1, z1, z, z, [z, z])
+    assert e.value.code == nb.EINVAL  # missing D_2, D_3
+    ctx.predict(100, 0.0, 4, z1, z1, z, z, [z, z])
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.force(idx, 10, 6, 1e-4, z, z, z, None, z1)
+    assert e.value.code == nb.ESTATE  # order above the predict's
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.force(idx, 10, 4, -1.0, z, z, None, None, z1)
+    assert e.value.code == nb.EINVAL
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.force(idx, 101, 4, 1e-4, z, z, None, None, z1)
+    assert e.value.code == nb.EINVAL
+    ctx.force(idx, 0, 4, 1e-4, None, None, None, None, None)  # n_act == 0: no-op
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.correct(idx, 10, 4, 0.1, 0.1, 0.3, 0.5, z1, z1, z, z, [z] * 4, z1, z, z, None, None, z1)
+    assert e.value.code == nb.EINVAL  # dt_min not a power of two
+    with pytest.raises(nb.NBodyError):
+        ctx.set_option("no_such_option", 1)
+    assert nb.strerror(nb.EINVAL) == "invalid argument" and nb.strerror(12345).startswith("unknown")
+    ctx.close()
+
+
+def test_force_host_matches_device_path(nb, O):
+    """Host-buffer entry point = same kernels: bit-identical to the device-pointer calls, and within tolerance
+    of the oracle."""
+    c = W.cluster(3, 2500)
+    n, order = c["n"], 6
+    D = U.oracle_bootstrap_derivs(c, 6)
+    t, dt = W.predictor_times(c["x"])
+    t_now = 2.0**-10
+    idx = W.active_list(n, 700, W.rng_for(3, 4))
+    ctx = nb.Context(n)
+    dev_out = U.gpu_force(ctx, n, order, c["eps2"], t_now, t, c["m"], c["x"], c["v"], D, idx)
+    na = idx.shape[0]
+    acc, jerk, snap, pot = np.zeros((na, 3)), np.zeros((na, 3)), np.zeros((na, 3)), np.zeros(na)
+    up, down = ctx.force_host(n, t_now, order, t, c["m"], c["x"], c["v"], D[:4], idx, na, c["eps2"], acc, jerk, snap,
+                              None, pot)
+    assert up == 8 * n * (2 + 6 + 12) + 4 * na and down == 8 * na * 10
+    assert np.array_equal(acc, dev_out[0]) and np.array_equal(jerk, dev_out[1])
+    assert np.array_equal(snap, dev_out[2]) and np.array_equal(pot, dev_out[4])
+    xp, vp, ap, jp = O.predict(t_now, order, t, c["x"], c["v"], D)
+    ref = O.force(c["m"], xp, vp, ap, jp, idx, order, c["eps2"])
+    U.check_force((acc, jerk, snap, None, pot), ref, order, "force_host")
+    ctx.close()
