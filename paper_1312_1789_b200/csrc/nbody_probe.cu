@@ -26,12 +26,18 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed) {
         for (int c = 0; c < kProbeChains; ++c) {
             if (KIND == 0) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[c]) : "f"(b), "f"(cc));
             if (KIND == 1) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(d[c]) : "d"(db));
-            if (KIND == 2) asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(f[c]) : "d"(d[c]));
+            if (KIND == 2) {  // dependent round trip fp64 -> fp32 -> fp64 (two conversions)
+                asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(f[c]) : "d"(d[c]));
+                asm volatile("cvt.f64.f32 %0, %1;" : "=d"(d[c]) : "f"(f[c]));
+            }
             if (KIND == 3) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f[c]));
-            if (KIND == 4) {
+            if (KIND == 4) {  // the literal difference pattern: DADD, F2F, and an FADD that consumes it
                 double t;
+                float g;
                 asm volatile("add.rn.f64 %0, %1, %2;" : "=d"(t) : "d"(d[c]), "d"(db));
-                asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(f[c]) : "d"(t));
+                asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(g) : "d"(t));
+                asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(f[c]) : "f"(g));
+                d[c] = t;
             }
         }
     }
@@ -54,7 +60,7 @@ int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
     NB_CUDA(c, cudaEventCreate(&e0));
     NB_CUDA(c, cudaEventCreate(&e1));
     const int grid = c->sm_count * 8;  // 2048 threads per SM
-    const double ops_per_launch = (double)grid * 256.0 * kProbeIters * kProbeChains * (kind == 4 ? 2.0 : 1.0);
+    const double ops_per_launch = (double)grid * 256.0 * kProbeIters * kProbeChains * (kind == 4 ? 3.0 : kind == 2 ? 2.0 : 1.0);
     double best = 0.0, spent = 0.0;
     int rc = NBODY_OK;
     for (int rep = 0; rep < 100000 && spent < (double)millis; ++rep) {

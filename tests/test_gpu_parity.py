@@ -7,7 +7,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 from paper_1312_1789_b200 import workloads as W
-from tests import gpu_util as U
+import gpu_util as U
 
 
 @pytest.fixture(scope="module")
