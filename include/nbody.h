@@ -158,7 +158,8 @@ int nbody_force_host(nbody_ctx *ctx, int64_t n, double t_now, int order,
 /* ------------------------------------------------------------------------------------------------------------
  * nbody_probe_peak -- chip micro-probes used for the roofline denominators.  Runs a
  * register-only loop of one instruction class on every SM for about `millis` ms and returns the achieved
- * rate in 1e12 thread-operations per second through *tera_ops_host (an FFMA counts as ONE operation).
+ * rate in 1e12 thread-operations per second in tera_ops_host[0] (an FFMA counts as ONE operation) and the SM
+ * clock in MHz measured inside that kernel (clock64 / globaltimer) in tera_ops_host[1]; HOST array of 2.
  *   kind 0 = FFMA (fp32), 1 = DADD (fp64 add), 2 = F2F (fp64->fp32->fp64 round trip, 2 ops), 3 = MUFU.RSQ,
  *   4 = the literal difference pattern DADD + F2F + FADD (3 ops).
  * Synchronises.

@@ -49,6 +49,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 
 __device__ __forceinline__ double u2d(unsigned lo, unsigned hi) { return __hiloint2double((int)hi, (int)lo); }
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
+// fp64 -> fp32, round to nearest even.  Written in PTX without .ftz: under -ftz=true the intrinsic would expand
+// to F2F + DSETP + predicated FMUL (denormal flush), 2 extra instructions per coordinate.
+__device__ __forceinline__ float d2f(double x) {
+    float r;
+    asm("cvt.rn.f32.f64 %0, %1;" : "=f"(r) : "d"(x));
+    return r;
+}
 __device__ __forceinline__ float frsqrt(float x) {
     float r;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -81,9 +88,9 @@ __device__ __forceinline__ void pair(const IPart<ORDER, DIFF> &I, const uint4 &q
     float d[3], dv[3], da[3], dj[3];
     float mj;
     if (DIFF == 0) {
-        d[0] = __double2float_rn(u2d(qa.x, qa.y) - I.x[0]);
-        d[1] = __double2float_rn(u2d(qa.z, qa.w) - I.x[1]);
-        d[2] = __double2float_rn(u2d(qb.x, qb.y) - I.x[2]);
+        d[0] = d2f(u2d(qa.x, qa.y) - I.x[0]);
+        d[1] = d2f(u2d(qa.z, qa.w) - I.x[1]);
+        d[2] = d2f(u2d(qb.x, qb.y) - I.x[2]);
     } else {
         d[0] = (u2f(qa.x) - I.xh[0]) + (u2f(qa.y) - I.xl[0]);
         d[1] = (u2f(qa.z) - I.xh[1]) + (u2f(qa.w) - I.xl[1]);

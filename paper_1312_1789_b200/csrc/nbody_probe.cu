@@ -10,7 +10,12 @@ constexpr int kProbeIters = 4096;
 constexpr int kProbeChains = 8;
 
 template <int KIND>
-__global__ void __launch_bounds__(256) k_probe(float *sink, float seed) {
+__global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned long long *clk) {
+    unsigned long long c0 = 0, g0 = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+        c0 = clock64();
+    }
     float f[kProbeChains];
     double d[kProbeChains];
 #pragma unroll
@@ -20,7 +25,7 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed) {
     }
     const float b = 0.999f + seed, cc = 1e-3f;
     const double db = 1e-3 + (double)seed;
-#pragma unroll 1
+#pragma unroll 8
     for (int it = 0; it < kProbeIters; ++it) {
 #pragma unroll
         for (int c = 0; c < kProbeChains; ++c) {
@@ -45,9 +50,16 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed) {
 #pragma unroll
     for (int c = 0; c < kProbeChains; ++c) s += f[c] + (float)d[c];
     if (s == 123.456f) sink[0] = s;  // never true in practice; keeps the chains live
+    if (blockIdx.x == 0 && threadIdx.x == 0) {  // SM cycles and nanoseconds this CTA ran: the SM clock under this load
+        unsigned long long g1;
+        const unsigned long long c1 = clock64();
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+        clk[0] = c1 - c0;
+        clk[1] = g1 - g0;
+    }
 }
 
-typedef void (*probe_fn)(float *, float);
+typedef void (*probe_fn)(float *, float, unsigned long long *);
 const probe_fn kProbes[5] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>};
 
 }  // namespace
@@ -55,7 +67,10 @@ const probe_fn kProbes[5] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_p
 int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
     NB_CUDA(c, cudaSetDevice(c->device));
     float *sink = nullptr;
-    NB_CUDA(c, cudaMalloc(&sink, sizeof(float)));
+    NB_CUDA(c, cudaMalloc(&sink, sizeof(float) + 2 * sizeof(unsigned long long) + 8));
+    unsigned long long *clk = reinterpret_cast<unsigned long long *>(reinterpret_cast<char *>(sink) + 8);
+    unsigned long long hclk[2] = {0, 0};
+    double best_mhz = 0.0;
     cudaEvent_t e0, e1;
     NB_CUDA(c, cudaEventCreate(&e0));
     NB_CUDA(c, cudaEventCreate(&e1));
@@ -65,7 +80,7 @@ int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
     int rc = NBODY_OK;
     for (int rep = 0; rep < 100000 && spent < (double)millis; ++rep) {
         cudaEventRecord(e0, 0);
-        kProbes[kind]<<<grid, 256>>>(sink, 0.0f);
+        kProbes[kind]<<<grid, 256>>>(sink, 0.0f, clk);
         c->launches += 1;
         cudaEventRecord(e1, 0);
         cudaError_t e = cudaEventSynchronize(e1);
@@ -75,13 +90,18 @@ int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
         spent += ms;
         if (rep > 0 && ms > 0.f) {
             const double rate = ops_per_launch / (ms * 1e-3) / 1e12;
-            if (rate > best) best = rate;
+            if (rate > best) {
+                best = rate;
+                if (cudaMemcpy(hclk, clk, sizeof(hclk), cudaMemcpyDeviceToHost) == cudaSuccess && hclk[1] > 0)
+                    best_mhz = (double)hclk[0] / (double)hclk[1] * 1e3;
+            }
         }
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
-    *tera_ops = best;
+    tera_ops[0] = best;
+    tera_ops[1] = best_mhz;
     return rc;
 }
 

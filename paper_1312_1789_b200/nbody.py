@@ -164,10 +164,11 @@ class Context:
                                           C.byref(up), C.byref(down)), "nbody_force_host")
         return up.value, down.value
 
-    def probe_peak(self, kind: int, millis: int = 200) -> float:
-        r = _dbl()
-        self._check(_lib.nbody_probe_peak(self._h, int(kind), int(millis), C.byref(r)), "nbody_probe_peak")
-        return r.value
+    def probe_peak(self, kind: int, millis: int = 200):
+        """Returns (1e12 thread-ops/s, SM MHz measured inside the probe kernel)."""
+        r = (_dbl * 2)()
+        self._check(_lib.nbody_probe_peak(self._h, int(kind), int(millis), r), "nbody_probe_peak")
+        return r[0], r[1]
 
     def launch_count(self) -> int:
         return int(_lib.nbody_launch_count(self._h))
