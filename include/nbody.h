@@ -57,6 +57,10 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
 /* Tuning / evidence knobs (host-side integers; unknown key -> NBODY_EINVAL).
  *   "diff_mode"   0 = literal: d = fl32(x_j - x_i), subtraction in fp64 (DADD + F2F)          [default]
  *                 1 = double-single: x = hi + lo (two fp32), d = (hi_j - hi_i) + (lo_j - lo_i)  (R10 note)
+ *   "dt_criterion_order" 0 = criterion of the scheme's own order p (R8)                        [default]
+ *                 4 | 6 = R8b: evaluate the same criterion family on the lowest 4 (6) derivatives only, i.e.
+ *                 dt = eta (A^(1)/A^(pc-2))^(1/(pc-3)) with pc = min(p, value).  pc = 4 is Aarseth's formula; for
+ *                 p = 8 it uses only a, j, s, c, all direct force-kernel outputs (no 1/h^k noise amplification).
  *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
  *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 4, 16, 64, 256)
  */

@@ -279,6 +279,10 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
  *        x1 = x0 + h/2 (v0+v1) + 3h^2/28 (a0-a1) + h^3/84 (j0+j1) + h^4/1680 (s0-s1)
  * c-7 interpolated a^(K..2K-1)(t1), Delta = a0 - a1 (formulas below).
  *
+ * c-8b: `crit_order` pc in {4, 6, 8}, pc < p, evaluates the c-8 criterion of order pc on a^(0..pc-1)(t1)
+ * (0 = order p).  Added after the CUDA path showed that with fp32 pair arithmetic (c-12) the interpolated
+ * a^(K..2K-1) of p >= 6 are rounding-noise dominated at small h and the order-p criterion collapses dt.
+ *
  * State arrays (in/out, [n][3] unless noted): t[n], dt[n], x, v, D[k] = a^(k)
  * for k = 0..p-1, pot_state[n].  Force arrays in active-list order [n_act][3].
  * ------------------------------------------------------------------------ */
@@ -287,9 +291,12 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                     double *t, double *dt, double *x, double *v, double *const *D,
                     double *pot_state,
                     const double *acc, const double *jerk, const double *snap,
-                    const double *crackle, const double *pot, int variant)
+                    const double *crackle, const double *pot, int variant, int crit_order)
 {
     const int p = order;
+    /* c-8b (R8b): the criterion may be evaluated on the lowest pc <= p derivatives only
+     * (crit_order 0 = p, the c-8 reading).  pc = 4 is Aarseth's formula on a, j, a2, a3. */
+    const int pc = (crit_order == 4 || crit_order == 6 || crit_order == 8) && crit_order < p ? crit_order : p;
 #pragma omp parallel for schedule(static)
     for (int64_t ia = 0; ia < n_act; ++ia) {
         const int64_t i = active_idx[ia];
@@ -347,7 +354,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
         }
         const double *dp[8];
         for (int k = 0; k < p; ++k) dp[k] = dnew[k];
-        const double dt_new = oracle_new_dt(p, dp, t_now, h, eta, dt_min, dt_max);
+        const double dt_new = oracle_new_dt(pc, dp, t_now, h, eta, dt_min, dt_max);
         for (int k = 0; k < p; ++k)
             for (int c = 0; c < 3; ++c) D[k][3 * i + c] = dnew[k][c];
         pot_state[i] = pot[ia];

@@ -200,6 +200,7 @@ struct CorrArgs {
     long long n_act;
     double t_now, eta, dt_min, dt_max;
     int k_min, k_max;
+    int crit_order;  // R8b: criterion evaluated on the lowest crit_order derivatives (<= ORDER)
     double *t, *dt, *x, *v, *D[8], *pot_state;
     const double *acc, *jerk, *snap, *crk, *pot;
 };
@@ -258,7 +259,13 @@ __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
         A.x[q] = x1;
         A.v[q] = v1;
     }
-    const double dt_new = new_dt<ORDER>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+    double dt_new;
+    if (ORDER >= 6 && A.crit_order == 4)
+        dt_new = new_dt<4>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+    else if (ORDER >= 8 && A.crit_order == 6)
+        dt_new = new_dt<6>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+    else
+        dt_new = new_dt<ORDER>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
 #pragma unroll
     for (int k = 0; k < ORDER; ++k)
 #pragma unroll
@@ -528,6 +535,11 @@ int nbody_set_option(nbody_ctx *h, const char *key, int64_t value) {
         c->force_split = (int)value;
         return NBODY_OK;
     }
+    if (!strcmp(key, "dt_criterion_order")) {
+        if (value != 0 && value != 4 && value != 6 && value != 8) return NBODY_EINVAL;
+        c->crit_order = (int)value;
+        return NBODY_OK;
+    }
     if (!strcmp(key, "force_lanes")) {
         if (value != 0 && value != 1 && value != 4 && value != 16 && value != 64 && value != 256) return NBODY_EINVAL;
         c->force_lanes = (int)value;
@@ -598,6 +610,7 @@ int nbody_correct(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int or
     CorrArgs A;
     A.idx = active_idx; A.n_act = n_act; A.t_now = t_now; A.eta = eta; A.dt_min = dt_min; A.dt_max = dt_max;
     A.k_min = kmin; A.k_max = kmax;
+    A.crit_order = (c->crit_order && c->crit_order < order) ? c->crit_order : order;
     A.t = t; A.dt = dt; A.x = x; A.v = v; A.pot_state = pot_state;
     for (int k = 0; k < 8; ++k) A.D[k] = k < order ? a_derivs[k] : nullptr;
     A.acc = acc; A.jerk = jerk; A.snap = snap; A.crk = crackle; A.pot = pot;

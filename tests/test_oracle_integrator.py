@@ -339,3 +339,48 @@ def test_block_timestep_energy_conservation_plummer(order):
     assert np.all(np.fmod(s.t, s.dt) == 0.0)
     e1 = OI.total_energy(s, eps2)
     assert abs((e1 - e0) / e0) < {4: 1e-6, 6: 1e-7, 8: 1e-7}[order]
+
+
+# ------------------------------------------------------------------------------------------- c-8b (R8b)
+@pytest.mark.parametrize("order,pc", [(6, 4), (8, 4), (8, 6)])
+def test_dt_criterion_order_option(order, pc):
+    """crit_order pc < p: the corrector's new step equals the order-pc criterion evaluated on the lowest pc
+    derivatives at t1 (which the corrector stores, so they can be read back), everything else is untouched;
+    it still reproduces eta/lambda on an exponential, and it differs from the order-p criterion in general."""
+    rng = np.random.default_rng(8)
+    n = 64
+    idx = np.arange(n, dtype=np.int32)
+    h = 2.0**-6
+    mk = lambda: np.ascontiguousarray(rng.normal(0, 1, (n, 3)))
+    base = dict(t=np.zeros(n), dt=np.full(n, h), x=mk(), v=mk(), D=[mk() * 3.0**k for k in range(8)], pot=np.zeros(n))
+    f = [mk() * 3.0**k for k in range(4)]
+    out = {}
+    for co in (0, pc):
+        s = dict(t=base["t"].copy(), dt=base["dt"].copy(), x=base["x"].copy(), v=base["v"].copy(),
+                 D=[d.copy() for d in base["D"]], pot=base["pot"].copy())
+        O.correct(idx, order, h, 0.1, 2.0**-30, 2.0**-2, s["t"], s["dt"], s["x"], s["v"], s["D"], s["pot"],
+                  f[0], f[1], f[2], f[3], np.zeros(n), crit_order=co)
+        out[co] = s
+    a, b = out[0], out[pc]
+    assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["v"], b["v"])
+    for k in range(order):
+        assert np.array_equal(a["D"][k], b["D"][k])
+    want_p = np.array([O.new_dt(order, [a["D"][k][i] for k in range(order)], h, h, 0.1, 2.0**-30, 2.0**-2) for i in range(n)])
+    want_pc = np.array([O.new_dt(pc, [a["D"][k][i] for k in range(pc)], h, h, 0.1, 2.0**-30, 2.0**-2) for i in range(n)])
+    assert np.array_equal(a["dt"], want_p)
+    assert np.array_equal(b["dt"], want_pc)
+    assert np.any(want_p != want_pc)
+
+
+def test_block_timestep_energy_conservation_criterion_order4():
+    """8th-order scheme stepped with Aarseth's four-derivative criterion (R8b): still lands on t_end and conserves
+    energy (fp64 oracle; the CUDA path needs this variant, R8b)."""
+    c = W.cluster(1, n=128)
+    eps2 = 1e-4
+    dt_min, dt_max = 2.0**-24, 2.0**-5
+    s = OI.bootstrap(c["m"], c["x"], c["v"], 8, eps2, dt_min=dt_min, dt_max=dt_max)
+    e0 = OI.total_energy(s, eps2)
+    OI.integrate(s, 0.125, eps2, 0.1, dt_min, dt_max, crit_order=4)
+    assert np.all(s.t == 0.125)
+    e1 = OI.total_energy(s, eps2)
+    assert abs((e1 - e0) / e0) < 1e-7
