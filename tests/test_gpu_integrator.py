@@ -137,14 +137,17 @@ def test_block_integration_vs_oracle(nb, O, order):
             dst.copy_(U.dev(src))
     agree = []
     for b in range(40):
+        if float(np.min(so.t + so.dt)) > DTMAX:
+            break
         sync()
         tn_o, idx_o = OI.block_step(so, eps2, 0.1, 2.0**-30, DTMAX, crit_order=CRIT)
         tn_g, na_g = g.block_step()
         assert tn_g == tn_o and na_g == idx_o.shape[0], "block %d differs" % b
         assert np.array_equal(g.active[:na_g].cpu().numpy(), idx_o)
         assert np.array_equal(g.t.cpu().numpy(), so.t)
-        assert np.max(np.abs(g.x.cpu().numpy() - so.x)) < 1e-11
-        assert np.max(np.abs(g.v.cpu().numpy() - so.v)) < 1e-9
+        # one step from identical states: |dv| <= h |da|, |da| <= 1e-5 |a| (force tolerance), h <= 2^-6, |a| <~ 1e2
+        assert np.max(np.abs(g.x.cpu().numpy() - so.x)) < 1e-10
+        assert np.max(np.abs(g.v.cpu().numpy() - so.v)) < 1e-8
         agree.append(np.mean(g.dt.cpu().numpy()[idx_o] == so.dt[idx_o]))
         gdt = g.dt.cpu().numpy()[idx_o]
         # every GPU step is a valid block step: power of two, in range, commensurate with the block time
@@ -153,7 +156,7 @@ def test_block_integration_vs_oracle(nb, O, order):
     # The step is a DECISION taken from a^(K..2K-1), which the corrector interpolates from differences of forces
     # divided by h^k: identical inputs give identical steps (test_correct_bit_exact); against the fp64 oracle the
     # mixed-precision forces move a decision only where dt_crit sits next to a power of two (R8b criterion).
-    assert np.mean(agree) > 0.9, np.mean(agree)
+    assert len(agree) >= 10 and np.mean(agree) > 0.9, (len(agree), np.mean(agree))
     # free-running: both integrate on their own to t = 1/64; trajectories stay close
     sync()
     OI.integrate(so, DTMAX, eps2, 0.1, 2.0**-30, DTMAX, crit_order=CRIT)
