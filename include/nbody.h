@@ -160,6 +160,19 @@ int nbody_force_host(nbody_ctx *ctx, int64_t n, double t_now, int order,
                      int64_t *h2d_bytes, int64_t *d2h_bytes);
 
 /* ------------------------------------------------------------------------------------------------------------
+ * nbody_step_host -- ONE WHOLE BLOCK STEP (a-1 .. a-4: selection, predict, force, correct) with HOST state: every
+ * pointer is a HOST pointer.  Copies t, dt, m, x, v, a_derivs[0..order-1], pot_state to ctx-owned staging, runs
+ * nbody_next_block + nbody_predict + nbody_force + nbody_correct (the same kernels), copies the updated t, dt, x, v,
+ * a_derivs[0..order-1], pot_state back IN PLACE and returns when they are in host memory.  *t_next_host and
+ * *n_act_host receive the block time and size.  a_derivs is a HOST array of 8 HOST pointers.  This is the call
+ * the end-to-end measurement times (host<->device copies inside the timed region).
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_step_host(nbody_ctx *ctx, int64_t n, int order, double eps2, double eta, double dt_min, double dt_max,
+                    double *t, double *dt, const double *m, double *x, double *v,
+                    double *const a_derivs[8] /* HOST array of HOST pointers */, double *pot_state,
+                    double *t_next_host, int64_t *n_act_host, int64_t *h2d_bytes, int64_t *d2h_bytes);
+
+/* ------------------------------------------------------------------------------------------------------------
  * nbody_probe_peak -- chip micro-probes used for the roofline denominators.  Runs a
  * register-only loop of one instruction class on every SM for about `millis` ms and returns the achieved
  * rate in 1e12 thread-operations per second in tera_ops_host[0] (an FFMA counts as ONE operation) and the SM

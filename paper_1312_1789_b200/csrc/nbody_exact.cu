@@ -750,3 +750,79 @@ extern "C" int nbody_force_host(nbody_ctx *h, int64_t n, double t_now, int order
     if (d2h_bytes) *d2h_bytes = down;
     return NBODY_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// One whole block step with HOST state (a-1 .. a-4): H2D of the state, selection, predict, force, correct,
+// D2H of the updated state.  Same kernels as the device-pointer calls.
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int nbody_step_host(nbody_ctx *h, int64_t n, int order, double eps2, double eta, double dt_min,
+                               double dt_max, double *t, double *dt, const double *m, double *x, double *v,
+                               double *const a_derivs[8], double *pot_state, double *t_next_host,
+                               int64_t *n_act_host, int64_t *h2d_bytes, int64_t *d2h_bytes) {
+    if (!h || (order != 4 && order != 6 && order != 8) || n < 1 || n > h->c.cap) return NBODY_EINVAL;
+    if (!t || !dt || !m || !x || !v || !a_derivs || !pot_state || !t_next_host || !n_act_host) return NBODY_EINVAL;
+    for (int k = 0; k < order; ++k)
+        if (!a_derivs[k]) return NBODY_EINVAL;
+    Ctx *c = &h->c;
+    NB_CUDA(c, cudaSetDevice(c->device));
+    const int K = order / 2;
+    // staging (doubles): t dt m pot [n] | x v [3n] | D[order][3n] | acc jerk snap crk [3n] fpot [n] | idx int32[n]
+    const size_t nd = (size_t)n * (4 + 6 + 3 * (size_t)order + 12 + 1);
+    const size_t need = nd * sizeof(double) + (size_t)n * sizeof(int32_t) + 256;
+    if (need > c->stage_bytes) {
+        NB_CUDA(c, cudaDeviceSynchronize());
+        cudaFree(c->stage);
+        c->stage = nullptr;
+        c->stage_bytes = 0;
+        NB_CUDA(c, cudaMalloc(&c->stage, need));
+        c->stage_bytes = need;
+    }
+    cudaStream_t st = 0;
+    double *d = (double *)c->stage;
+    double *d_t = d, *d_dt = d + n, *d_m = d + 2 * n, *d_pot = d + 3 * n, *d_x = d + 4 * n, *d_v = d + 7 * n;
+    double *d_D[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    for (int k = 0; k < order; ++k) d_D[k] = d + 10 * n + (size_t)k * 3 * n;
+    double *o = d + 10 * n + (size_t)order * 3 * n;
+    double *o_acc = o, *o_jerk = o + 3 * n, *o_snap = o + 6 * n, *o_crk = o + 9 * n, *o_pot = o + 12 * n;
+    int32_t *d_idx = (int32_t *)(o + 13 * n);
+    int64_t up = 0, down = 0;
+    auto h2d = [&](double *dst, const double *src, size_t cnt) {
+        up += (int64_t)(cnt * sizeof(double));
+        return cudaMemcpyAsync(dst, src, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
+    };
+    auto d2h = [&](double *dst, const double *src, size_t cnt) {
+        down += (int64_t)(cnt * sizeof(double));
+        return cudaMemcpyAsync(dst, src, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
+    };
+    NB_CUDA(c, h2d(d_t, t, n));
+    NB_CUDA(c, h2d(d_dt, dt, n));
+    NB_CUDA(c, h2d(d_m, m, n));
+    NB_CUDA(c, h2d(d_pot, pot_state, n));
+    NB_CUDA(c, h2d(d_x, x, 3 * n));
+    NB_CUDA(c, h2d(d_v, v, 3 * n));
+    for (int k = 0; k < order; ++k) NB_CUDA(c, h2d(d_D[k], a_derivs[k], 3 * n));
+    double t_next = 0.0;
+    int64_t n_act = 0;
+    int rc = nbody_next_block(h, n, d_t, d_dt, d_idx, &t_next, &n_act, st);
+    if (rc != NBODY_OK) return rc;
+    rc = nbody_predict(h, n, t_next, order, d_t, d_m, d_x, d_v, d_D, st);
+    if (rc != NBODY_OK) return rc;
+    rc = nbody_force(h, d_idx, n_act, order, eps2, o_acc, o_jerk, K >= 3 ? o_snap : nullptr, K >= 4 ? o_crk : nullptr,
+                     o_pot, st);
+    if (rc != NBODY_OK) return rc;
+    rc = nbody_correct(h, d_idx, n_act, order, t_next, eta, dt_min, dt_max, d_t, d_dt, d_x, d_v, d_D, d_pot, o_acc,
+                       o_jerk, K >= 3 ? o_snap : nullptr, K >= 4 ? o_crk : nullptr, o_pot, st);
+    if (rc != NBODY_OK) return rc;
+    NB_CUDA(c, d2h(t, d_t, n));
+    NB_CUDA(c, d2h(dt, d_dt, n));
+    NB_CUDA(c, d2h(pot_state, d_pot, n));
+    NB_CUDA(c, d2h(x, d_x, 3 * n));
+    NB_CUDA(c, d2h(v, d_v, 3 * n));
+    for (int k = 0; k < order; ++k) NB_CUDA(c, d2h(a_derivs[k], d_D[k], 3 * n));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    *t_next_host = t_next;
+    *n_act_host = n_act;
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return NBODY_OK;
+}

@@ -41,6 +41,8 @@ SIGNATURES = {
     "nbody_get_predicted": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "nbody_force_host": (C.c_int, [_vp, _i64, _dbl, C.c_int, _vp, _vp, _vp, _vp, C.POINTER(_vp), _vp, _i64, _dbl,
                                    _vp, _vp, _vp, _vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
+    "nbody_step_host": (C.c_int, [_vp, _i64, C.c_int, _dbl, _dbl, _dbl, _dbl, _vp, _vp, _vp, _vp, _vp, C.POINTER(_vp),
+                                  _vp, C.POINTER(_dbl), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
     "nbody_probe_peak": (C.c_int, [_vp, C.c_int, C.c_int, C.POINTER(_dbl)]),
     "nbody_launch_count": (_i64, [_vp]),
     "nbody_last_force_geometry": (C.c_int, [_vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
@@ -163,6 +165,15 @@ class Context:
                                           _ptr(acc), _ptr(jerk), _ptr(snap), _ptr(crackle), _ptr(pot),
                                           C.byref(up), C.byref(down)), "nbody_force_host")
         return up.value, down.value
+
+    def step_host(self, n, order, eps2, eta, dt_min, dt_max, t, dt, m, x, v, a_derivs, pot_state):
+        """One whole block step on HOST (numpy) state, in place; returns (t_next, n_act, h2d_bytes, d2h_bytes)."""
+        tn, na, up, down = _dbl(), _i64(), _i64(), _i64()
+        self._check(_lib.nbody_step_host(self._h, int(n), int(order), float(eps2), float(eta), float(dt_min),
+                                         float(dt_max), _ptr(t), _ptr(dt), _ptr(m), _ptr(x), _ptr(v),
+                                         _ptr_array(a_derivs, 8), _ptr(pot_state), C.byref(tn), C.byref(na),
+                                         C.byref(up), C.byref(down)), "nbody_step_host")
+        return tn.value, na.value, up.value, down.value
 
     def probe_peak(self, kind: int, millis: int = 200):
         """Returns (1e12 thread-ops/s, SM MHz measured inside the probe kernel)."""
