@@ -1,22 +1,35 @@
-// libnbody.so, translation unit 2: K_force (a-3), K_reduce (a-3b) and the peak micro-probes.
+// libnbody.so, translation unit 2: K_force (a-3) and K_reduce (a-3b).
 //
 // K_force computes, for each active i, the sums of DESIGN.md R1 (= SURVEY.md c-1; the paper prints no formula,
 // PAPER.md:15/:43 name the scheme, PAPER.md:31 the mixed precision) over the packed j-store:
-//   - i-particles live in registers (R per thread), j-tiles of kTileJ particles are staged plane by plane into
-//     shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier) through a kStages-deep ring;
-//   - d = fl32(x_j - x_i) with the subtraction in fp64 (DIFF 0) or double-single (DIFF 1); all pair arithmetic
-//     fp32 with MUFU.RSQ; fp32 partial sums over <= 64 consecutive j, then fp64 accumulators (R10);
-//   - the self pair is excluded by index (R2), but the compare/select is only executed by warps whose
-//     i-indices fall inside the current j-tile (warp-uniform branch), so the main loop is mask-free;
-//   - a CTA is IT = 256/JL i-lanes x JL j-lanes: JL = 1 for big blocks (every lane reads the same j: smem
-//     broadcast), JL up to 256 for tiny blocks (lanes share one i and stride over j), reduced through smem;
-//   - gridDim.y = S j-splits; S > 1 writes fp64 partials [S][NC][n_act] that K_reduce sums in fixed order.
+//   - every thread owns TWO i-particles and runs the fp32 pair arithmetic on both at once with Blackwell's packed
+//     f32x2 instructions (PTX fma/mul/add.f32x2 -> SASS FFMA2 / FMUL2 / FADD2): lane 0 = first i, lane 1 = second i.
+//     The scalar form is limited by issue slots and by register-file bandwidth (a 3-source FFMA with two sources in
+//     the same register bank takes 2 cycles); the packed form reads aligned 64-bit register pairs and halves the
+//     instruction count of the fp32 part.  The j operand of a packed instruction is the broadcast pair {v, v},
+//     which is why the j-store keeps fp32 values twice (nbody_internal.h);
+//   - j-tiles of kTileJ particles are staged plane by plane into shared memory by 1-D TMA bulk copies
+//     (cp.async.bulk + mbarrier) through a ring; every pair-loop read is an LDS.128 broadcast;
+//   - d = fl32(x_j - x_i) with the subtraction in fp64 (DIFF 0: DADD + F2F per lane) or double-single (DIFF 1:
+//     packed fp32 adds of hi and lo parts); MUFU.RSQ per lane; fp32 partial sums over <= 64 consecutive j, then
+//     fp64 accumulators, which live in shared memory (one slot per thread and component) to free registers (R10);
+//   - the self pair is excluded by index (R2), but the compare/select is only executed by warps whose i-indices
+//     fall inside the current j-tile (warp-uniform branch), so the main loop is mask-free;
+//   - a CTA is IT = 256/JL i-lanes x JL j-lanes (2 IT i-particles): JL = 1 for big blocks (every lane reads the
+//     same j: smem broadcast), JL up to 256 for tiny blocks; the j-lanes are reduced through shared memory in
+//     fixed order; gridDim.y = S j-splits; S > 1 writes fp64 partials [S][NC][n_act] that K_reduce sums in order.
 #include <math.h>
 
 #include "nbody_internal.h"
 
+#ifndef NB_UNROLL
+#define NB_UNROLL 2
+#endif
+
 namespace nbody {
 namespace {
+
+constexpr int kUnroll = NB_UNROLL;  // j-particles per unrolled group of the pair loop
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -47,6 +60,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         : "memory");
 }
 
+// ---- scalar helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ double u2d(unsigned lo, unsigned hi) { return __hiloint2double((int)hi, (int)lo); }
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
 // fp64 -> fp32, round to nearest even.  Written in PTX without .ftz: under -ftz=true the intrinsic would expand
@@ -62,8 +76,50 @@ __device__ __forceinline__ float frsqrt(float x) {
     return r;
 }
 
+// ---- packed f32x2 (one 64-bit register pair = {lane 0, lane 1}) -----------------------------------------
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float a, float b) {
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ f2 pku(unsigned a, unsigned b) {
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ void upk(f2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) {
+    f2 r;
+    asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) {
+    f2 r;
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) {
+    f2 r;
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+template <int ORDER, int DIFF>
+struct Geo {
+    static constexpr int K = ORDER / 2;
+    static constexpr int NC = 3 * K + 1;                        // components per i: 3K vectors + pot
+    static constexpr int XP = DIFF ? 3 : 1;                     // position planes (P0 | D0, D1, D2)
+    static constexpr int NQ = XP + (ORDER == 4 ? 3 : ORDER == 6 ? 4 : 6);  // planes staged per tile
+    static constexpr int STAGES = NQ >= 7 ? 3 : 4;              // TMA ring depth
+    static constexpr uint32_t STAGE_BYTES = NQ * kTileJ * 16;
+    static constexpr size_t TILE_BYTES = (size_t)STAGES * STAGE_BYTES;
+    static constexpr size_t ACC_BYTES = (size_t)2 * NC * kThreads * sizeof(double);
+    static constexpr size_t SMEM = TILE_BYTES + ACC_BYTES + 64;  // + mbarriers
+};
+
 struct ForceArgs {
-    const uint4 *q[4];  // planes in use: {Q0,Q1,Q2,Q3} (DIFF 0) or {Q4,Q5,Q2,Q3} (DIFF 1)
+    const uint4 *q[9];  // planes in kernel order: position planes, then P1, P2, ...
     const int32_t *idx;
     int n_act;
     int n_tiles;
@@ -74,144 +130,162 @@ struct ForceArgs {
 };
 
 template <int ORDER, int DIFF>
-struct IPart {  // one i-particle in registers
-    double x[3];
-    float xh[3], xl[3];
-    float v[3], a[3], j[3];
-    int idx;
+struct IPair {          // the thread's two i-particles
+    double x[2][3];     // DIFF 0
+    f2 nxh[3], nxl[3];  // DIFF 1: negated hi and lo parts
+    f2 nv[3], na[3], nj[3];  // negated, so that a difference is one packed add
+    int idx[2];
 };
 
-// One pair: accumulates into pa[0 .. 3K] (pot as +m/r, negated at the end).
+struct Consts {  // loop-invariant packed constants
+    f2 eps2, m3, three, m4;
+};
+
+// One j against the thread's two i-particles; accumulates into pa[0 .. 3K] (pot as +m/r, negated at the end).
+// tq = base of the staged tile (plane p at tq + p * kTileJ), jt = index inside the tile.
 template <int ORDER, int DIFF, bool MASK>
-__device__ __forceinline__ void pair(const IPart<ORDER, DIFF> &I, const uint4 &qa, const uint4 &qb, const uint4 &qc,
-                                     const uint4 &qd, int jglob, float eps2, float *pa) {
-    float d[3], dv[3], da[3], dj[3];
-    float mj;
+__device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *tq, int jt, int jglob,
+                                      const Consts &C, f2 *pa) {
+    typedef Geo<ORDER, DIFF> G;
+    constexpr int XP = G::XP;
+    f2 d[3];
+    const uint4 qb = tq[XP * kTileJ + jt];  // P1 = { z (f64), m, m }
     if (DIFF == 0) {
-        d[0] = d2f(u2d(qa.x, qa.y) - I.x[0]);
-        d[1] = d2f(u2d(qa.z, qa.w) - I.x[1]);
-        d[2] = d2f(u2d(qb.x, qb.y) - I.x[2]);
+        const uint4 qa = tq[jt];  // P0 = { x, y }
+        const double xj = u2d(qa.x, qa.y), yj = u2d(qa.z, qa.w), zj = u2d(qb.x, qb.y);
+        d[0] = pk(d2f(xj - I.x[0][0]), d2f(xj - I.x[1][0]));
+        d[1] = pk(d2f(yj - I.x[0][1]), d2f(yj - I.x[1][1]));
+        d[2] = pk(d2f(zj - I.x[0][2]), d2f(zj - I.x[1][2]));
     } else {
-        d[0] = (u2f(qa.x) - I.xh[0]) + (u2f(qa.y) - I.xl[0]);
-        d[1] = (u2f(qa.z) - I.xh[1]) + (u2f(qa.w) - I.xl[1]);
-        d[2] = (u2f(qb.x) - I.xh[2]) + (u2f(qb.y) - I.xl[2]);
-    }
-    mj = u2f(qb.z);
-    dv[0] = u2f(qb.w) - I.v[0];
-    dv[1] = u2f(qc.x) - I.v[1];
-    dv[2] = u2f(qc.y) - I.v[2];
-    float r2 = fmaf(d[0], d[0], eps2);
-    r2 = fmaf(d[1], d[1], r2);
-    r2 = fmaf(d[2], d[2], r2);
-    float rv = d[0] * dv[0];
-    rv = fmaf(d[1], dv[1], rv);
-    rv = fmaf(d[2], dv[2], rv);
-    float rinv = frsqrt(r2);
-    if (MASK) rinv = (jglob == I.idx) ? 0.f : rinv;
-    const float rinv2 = rinv * rinv;
-    const float mrinv = mj * rinv;
-    const float q = mrinv * rinv2;
-    const float alpha = rv * rinv2;
-    constexpr int K = ORDER / 2;
-    pa[3 * K] += mrinv;
-    const float c1 = -3.f * alpha;
-    float Jp[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        Jp[c] = fmaf(c1, d[c], dv[c]);
-        pa[c] = fmaf(q, d[c], pa[c]);
-        pa[3 + c] = fmaf(q, Jp[c], pa[3 + c]);
-    }
-    if (ORDER >= 6) {
-        da[0] = u2f(qc.z) - I.a[0];
-        da[1] = u2f(qc.w) - I.a[1];
-        da[2] = u2f(qd.x) - I.a[2];
-        float w = dv[0] * dv[0];
-        w = fmaf(dv[1], dv[1], w);
-        w = fmaf(dv[2], dv[2], w);
-        w = fmaf(d[0], da[0], w);
-        w = fmaf(d[1], da[1], w);
-        w = fmaf(d[2], da[2], w);
-        const float beta = fmaf(alpha, alpha, w * rinv2);
-        const float c2 = c1 + c1;
-        const float c3 = -3.f * beta;
-        float Sp[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            Sp[c] = fmaf(c3, d[c], fmaf(c2, Jp[c], da[c]));
-            pa[6 + c] = fmaf(q, Sp[c], pa[6 + c]);
+            const uint4 qx = tq[c * kTileJ + jt];  // Dc = { hi, hi, lo, lo }
+            d[c] = add2(add2(pku(qx.x, qx.y), I.nxh[c]), add2(pku(qx.z, qx.w), I.nxl[c]));
+        }
+    }
+    const f2 mj = pku(qb.z, qb.w);
+    const uint4 qc = tq[(XP + 1) * kTileJ + jt];  // P2 = { vx, vx, vy, vy }
+    const uint4 qd = tq[(XP + 2) * kTileJ + jt];  // P3 = { vz, vz, ax, ax }
+    f2 dv[3], da[3], dj[3];
+    dv[0] = add2(pku(qc.x, qc.y), I.nv[0]);
+    dv[1] = add2(pku(qc.z, qc.w), I.nv[1]);
+    dv[2] = add2(pku(qd.x, qd.y), I.nv[2]);
+    f2 r2 = fma2(d[0], d[0], C.eps2);
+    r2 = fma2(d[1], d[1], r2);
+    r2 = fma2(d[2], d[2], r2);
+    f2 rv = mul2(d[0], dv[0]);
+    rv = fma2(d[1], dv[1], rv);
+    rv = fma2(d[2], dv[2], rv);
+    float r0, r1;
+    upk(r2, r0, r1);
+    r0 = frsqrt(r0);
+    r1 = frsqrt(r1);
+    if (MASK) {
+        r0 = (jglob == I.idx[0]) ? 0.f : r0;
+        r1 = (jglob == I.idx[1]) ? 0.f : r1;
+    }
+    const f2 rinv = pk(r0, r1);
+    const f2 rinv2 = mul2(rinv, rinv);
+    const f2 mrinv = mul2(mj, rinv);
+    const f2 q = mul2(mrinv, rinv2);
+    const f2 alpha = mul2(rv, rinv2);
+    constexpr int K = ORDER / 2;
+    pa[3 * K] = add2(pa[3 * K], mrinv);
+    const f2 c1 = mul2(C.m3, alpha);
+    f2 Jp[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        Jp[c] = fma2(c1, d[c], dv[c]);
+        pa[c] = fma2(q, d[c], pa[c]);
+        pa[3 + c] = fma2(q, Jp[c], pa[3 + c]);
+    }
+    if (ORDER >= 6) {
+        const uint4 qe = tq[(XP + 3) * kTileJ + jt];  // P4 = { ay, ay, az, az }
+        da[0] = add2(pku(qd.z, qd.w), I.na[0]);
+        da[1] = add2(pku(qe.x, qe.y), I.na[1]);
+        da[2] = add2(pku(qe.z, qe.w), I.na[2]);
+        f2 w = mul2(dv[0], dv[0]);
+        w = fma2(dv[1], dv[1], w);
+        w = fma2(dv[2], dv[2], w);
+        w = fma2(d[0], da[0], w);
+        w = fma2(d[1], da[1], w);
+        w = fma2(d[2], da[2], w);
+        const f2 beta = fma2(alpha, alpha, mul2(w, rinv2));
+        const f2 c2 = add2(c1, c1);
+        const f2 c3 = mul2(C.m3, beta);
+        f2 Sp[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Sp[c] = fma2(c3, d[c], fma2(c2, Jp[c], da[c]));
+            pa[6 + c] = fma2(q, Sp[c], pa[6 + c]);
         }
         if (ORDER >= 8) {
-            dj[0] = u2f(qd.y) - I.j[0];
-            dj[1] = u2f(qd.z) - I.j[1];
-            dj[2] = u2f(qd.w) - I.j[2];
-            float va = dv[0] * da[0];
-            va = fmaf(dv[1], da[1], va);
-            va = fmaf(dv[2], da[2], va);
-            float g = 3.f * va;
-            g = fmaf(d[0], dj[0], g);
-            g = fmaf(d[1], dj[1], g);
-            g = fmaf(d[2], dj[2], g);
+            const uint4 qf = tq[(XP + 4) * kTileJ + jt];  // P5 = { jx, jx, jy, jy }
+            const uint4 qg = tq[(XP + 5) * kTileJ + jt];  // P6 = { jz, jz, 0, 0 }
+            dj[0] = add2(pku(qf.x, qf.y), I.nj[0]);
+            dj[1] = add2(pku(qf.z, qf.w), I.nj[1]);
+            dj[2] = add2(pku(qg.x, qg.y), I.nj[2]);
+            f2 va = mul2(dv[0], da[0]);
+            va = fma2(dv[1], da[1], va);
+            va = fma2(dv[2], da[2], va);
+            f2 g = mul2(C.three, va);
+            g = fma2(d[0], dj[0], g);
+            g = fma2(d[1], dj[1], g);
+            g = fma2(d[2], dj[2], g);
             // gamma = g / s2 + alpha (3 beta - 4 alpha^2)
-            const float t = fmaf(-4.f * alpha, alpha, 3.f * beta);
-            const float gamma = fmaf(alpha, t, g * rinv2);
-            const float c4 = 3.f * c1;   // -9 alpha
-            const float c5 = 3.f * c3;   // -9 beta
-            const float c6 = -3.f * gamma;
+            const f2 t = fma2(mul2(C.m4, alpha), alpha, mul2(C.three, beta));
+            const f2 gamma = fma2(alpha, t, mul2(g, rinv2));
+            const f2 c4 = mul2(C.three, c1);  // -9 alpha
+            const f2 c5 = mul2(C.three, c3);  // -9 beta
+            const f2 c6 = mul2(C.m3, gamma);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float Cp = fmaf(c6, d[c], fmaf(c5, Jp[c], fmaf(c4, Sp[c], dj[c])));
-                pa[9 + c] = fmaf(q, Cp, pa[9 + c]);
+                const f2 Cp = fma2(c6, d[c], fma2(c5, Jp[c], fma2(c4, Sp[c], dj[c])));
+                pa[9 + c] = fma2(q, Cp, pa[9 + c]);
             }
         }
     }
 }
 
-template <int ORDER, int R, int JL, int DIFF, bool MASK>
-__device__ __forceinline__ void tile_compute(const IPart<ORDER, DIFF> (&I)[R], const uint4 *tq, int j0, int jl,
-                                             float eps2, float (&pa)[R][3 * (ORDER / 2) + 1],
-                                             double (&acc)[R][3 * (ORDER / 2) + 1]) {
-    constexpr int NQ = ORDER == 4 ? 3 : 4;
-    constexpr int NC = 3 * (ORDER / 2) + 1;
+// fp32 partials -> the thread's fp64 accumulator slots in shared memory: acc[(2 c + lane) * kThreads + tid]
+template <int NC>
+__device__ __forceinline__ void flush(f2 (&pa)[NC], double *acc_mine) {
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        float a, b;
+        upk(pa[c], a, b);
+        acc_mine[(2 * c) * kThreads] += (double)a;
+        acc_mine[(2 * c + 1) * kThreads] += (double)b;
+        pa[c] = 0ull;
+    }
+}
+
+template <int ORDER, int JL, int DIFF, bool MASK>
+__device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const uint4 *tq, int j0, int jl,
+                                             const Consts &C, f2 (&pa)[3 * (ORDER / 2) + 1], double *acc_mine) {
     constexpr int JPT = kTileJ / JL;
     constexpr int CH = JPT < 64 ? JPT : 64;
 #pragma unroll 1
     for (int jj0 = 0; jj0 < JPT; jj0 += CH) {
-#pragma unroll 4
+#pragma unroll kUnroll
         for (int u = 0; u < CH; ++u) {
             const int jt = (jj0 + u) * JL + jl;
-            const uint4 qa = tq[jt];
-            const uint4 qb = tq[kTileJ + jt];
-            const uint4 qc = tq[2 * kTileJ + jt];
-            uint4 qd = make_uint4(0, 0, 0, 0);
-            if (NQ == 4) qd = tq[3 * kTileJ + jt];
-#pragma unroll
-            for (int r = 0; r < R; ++r) pair<ORDER, DIFF, MASK>(I[r], qa, qb, qc, qd, j0 + jt, eps2, pa[r]);
+            pair2<ORDER, DIFF, MASK>(I, tq, jt, j0 + jt, C, pa);
         }
-        if (JPT >= 64) {
-#pragma unroll
-            for (int r = 0; r < R; ++r)
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    acc[r][c] += (double)pa[r][c];
-                    pa[r][c] = 0.f;
-                }
-        }
+        if (JPT >= 64) flush(pa, acc_mine);
     }
 }
 
-template <int ORDER, int R, int JL, int DIFF>
+template <int ORDER, int JL, int DIFF>
 __global__ void __launch_bounds__(kThreads, 2) k_force(const ForceArgs A) {
-    constexpr int NQ = ORDER == 4 ? 3 : 4;
-    constexpr int K = ORDER / 2;
-    constexpr int NC = 3 * K + 1;
-    constexpr int IT = kThreads / JL;
-    constexpr int JPT = kTileJ / JL;
-    constexpr uint32_t kStageBytes = NQ * kTileJ * 16;
-    static_assert(JL == 1 || R == 1, "j-lanes only with one i per thread");
+    typedef Geo<ORDER, DIFF> G;
+    constexpr int NQ = G::NQ, NC = G::NC, XP = G::XP, STAGES = G::STAGES;
+    constexpr int IT = kThreads / JL;    // threads per j-lane; the CTA owns 2 IT i-particles
+    constexpr int JPT = kTileJ / JL;     // j-particles per thread and tile
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint4 *tiles = reinterpret_cast<uint4 *>(smem_raw);
-    const uint32_t bar0 = smem_u32(smem_raw + kStages * kStageBytes);
+    double *acc_sm = reinterpret_cast<double *>(smem_raw + G::TILE_BYTES);
+    const uint32_t bar0 = smem_u32(smem_raw + G::TILE_BYTES + G::ACC_BYTES);
     const int tid = threadIdx.x;
     const int il = tid % IT, jl = tid / IT;
     const int tile_lo = (int)((long long)A.n_tiles * blockIdx.y / A.splits);
@@ -220,129 +294,127 @@ __global__ void __launch_bounds__(kThreads, 2) k_force(const ForceArgs A) {
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(bar0 + 8 * s, 1);
+        for (int s = 0; s < STAGES; ++s) mbar_init(bar0 + 8 * s, 1);
         mbar_fence_init();
     }
     __syncthreads();
     auto issue = [&](int k) {  // k = tile number within this CTA's range
-        const int s = k % kStages;
+        const int s = k % STAGES;
         const uint32_t bar = bar0 + 8 * s;
-        mbar_expect_tx(bar, kStageBytes);
+        mbar_expect_tx(bar, G::STAGE_BYTES);
         const size_t off = (size_t)(tile_lo + k) * kTileJ;
 #pragma unroll
         for (int p = 0; p < NQ; ++p)
             bulk_g2s(smem_u32(tiles + (s * NQ + p) * kTileJ), A.q[p] + off, kTileJ * 16, bar);
     };
     if (tid == 0) {
-        for (int k = 0; k < kStages - 1 && k < ntile; ++k) issue(k);
+        for (int k = 0; k < STAGES - 1 && k < ntile; ++k) issue(k);
     }
 
-    // ---- i-particles into registers ----
-    IPart<ORDER, DIFF> I[R];
-    float pa[R][NC];
-    double acc[R][NC];
+    // ---- the thread's two i-particles into registers (gathered from the same j-store: R4) ----
+    IPair<ORDER, DIFF> I;
+    float nv[2][3], na[2][3], nj[2][3], xh[2][3], xl[2][3];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int slot = blockIdx.x * (IT * R) + r * IT + il;
+    for (int r = 0; r < 2; ++r) {
+        const int slot = blockIdx.x * (2 * IT) + r * IT + il;
         const bool valid = slot < A.n_act;
         const int gi = A.idx[valid ? slot : A.n_act - 1];
-        I[r].idx = valid ? gi : -1;
-        const uint4 qa = __ldg(A.q[0] + gi), qb = __ldg(A.q[1] + gi), qc = __ldg(A.q[2] + gi);
+        I.idx[r] = valid ? gi : -1;
+        const uint4 qb = __ldg(A.q[XP] + gi), qc = __ldg(A.q[XP + 1] + gi), qd = __ldg(A.q[XP + 2] + gi);
         if (DIFF == 0) {
-            I[r].x[0] = u2d(qa.x, qa.y);
-            I[r].x[1] = u2d(qa.z, qa.w);
-            I[r].x[2] = u2d(qb.x, qb.y);
+            const uint4 qa = __ldg(A.q[0] + gi);
+            I.x[r][0] = u2d(qa.x, qa.y);
+            I.x[r][1] = u2d(qa.z, qa.w);
+            I.x[r][2] = u2d(qb.x, qb.y);
         } else {
-            I[r].xh[0] = u2f(qa.x); I[r].xl[0] = u2f(qa.y);
-            I[r].xh[1] = u2f(qa.z); I[r].xl[1] = u2f(qa.w);
-            I[r].xh[2] = u2f(qb.x); I[r].xl[2] = u2f(qb.y);
-        }
-        I[r].v[0] = u2f(qb.w);
-        I[r].v[1] = u2f(qc.x);
-        I[r].v[2] = u2f(qc.y);
-        if (ORDER >= 6) {
-            const uint4 qd = __ldg(A.q[3] + gi);
-            I[r].a[0] = u2f(qc.z);
-            I[r].a[1] = u2f(qc.w);
-            I[r].a[2] = u2f(qd.x);
-            I[r].j[0] = u2f(qd.y);
-            I[r].j[1] = u2f(qd.z);
-            I[r].j[2] = u2f(qd.w);
-        }
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            pa[r][c] = 0.f;
-            acc[r][c] = 0.0;
+            for (int c = 0; c < 3; ++c) {
+                const uint4 qx = __ldg(A.q[c] + gi);
+                xh[r][c] = -u2f(qx.x);
+                xl[r][c] = -u2f(qx.z);
+            }
         }
+        nv[r][0] = -u2f(qc.x);
+        nv[r][1] = -u2f(qc.z);
+        nv[r][2] = -u2f(qd.x);
+        if (ORDER >= 6) {
+            const uint4 qe = __ldg(A.q[XP + 3] + gi);
+            na[r][0] = -u2f(qd.z);
+            na[r][1] = -u2f(qe.x);
+            na[r][2] = -u2f(qe.z);
+        }
+        if (ORDER >= 8) {
+            const uint4 qf = __ldg(A.q[XP + 4] + gi), qg = __ldg(A.q[XP + 5] + gi);
+            nj[r][0] = -u2f(qf.x);
+            nj[r][1] = -u2f(qf.z);
+            nj[r][2] = -u2f(qg.x);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        I.nv[c] = pk(nv[0][c], nv[1][c]);
+        if (ORDER >= 6) I.na[c] = pk(na[0][c], na[1][c]);
+        if (ORDER >= 8) I.nj[c] = pk(nj[0][c], nj[1][c]);
+        if (DIFF == 1) {
+            I.nxh[c] = pk(xh[0][c], xh[1][c]);
+            I.nxl[c] = pk(xl[0][c], xl[1][c]);
+        }
+    }
+    Consts C;
+    C.eps2 = pk(A.eps2, A.eps2);
+    C.m3 = pk(-3.f, -3.f);
+    C.three = pk(3.f, 3.f);
+    C.m4 = pk(-4.f, -4.f);
+    f2 pa[NC];
+    double *acc_mine = acc_sm + tid;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        pa[c] = 0ull;
+        acc_mine[(2 * c) * kThreads] = 0.0;
+        acc_mine[(2 * c + 1) * kThreads] = 0.0;
     }
 
     // ---- main loop over this CTA's j-tiles ----
     int since = 0;
 #pragma unroll 1
     for (int k = 0; k < ntile; ++k) {
-        const int s = k % kStages;
+        const int s = k % STAGES;
         __syncthreads();  // every warp is done with tile k-1, whose stage is refilled now
-        if (tid == 0 && k + kStages - 1 < ntile) issue(k + kStages - 1);
-        mbar_wait(bar0 + 8 * s, (uint32_t)((k / kStages) & 1));
+        if (tid == 0 && k + STAGES - 1 < ntile) issue(k + STAGES - 1);
+        mbar_wait(bar0 + 8 * s, (uint32_t)((k / STAGES) & 1));
         const uint4 *tq = tiles + s * NQ * kTileJ;
         const int j0 = (tile_lo + k) * kTileJ;
-        bool mine = false;
-#pragma unroll
-        for (int r = 0; r < R; ++r) mine |= (unsigned)(I[r].idx - j0) < (unsigned)kTileJ;
+        const bool mine = (unsigned)(I.idx[0] - j0) < (unsigned)kTileJ || (unsigned)(I.idx[1] - j0) < (unsigned)kTileJ;
         if (__any_sync(0xffffffffu, mine))
-            tile_compute<ORDER, R, JL, DIFF, true>(I, tq, j0, jl, A.eps2, pa, acc);
+            tile_compute<ORDER, JL, DIFF, true>(I, tq, j0, jl, C, pa, acc_mine);
         else
-            tile_compute<ORDER, R, JL, DIFF, false>(I, tq, j0, jl, A.eps2, pa, acc);
+            tile_compute<ORDER, JL, DIFF, false>(I, tq, j0, jl, C, pa, acc_mine);
         if (JPT < 64) {
             if (++since == 64 / JPT) {
                 since = 0;
-#pragma unroll
-                for (int r = 0; r < R; ++r)
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) {
-                        acc[r][c] += (double)pa[r][c];
-                        pa[r][c] = 0.f;
-                    }
+                flush(pa, acc_mine);
             }
         }
     }
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-#pragma unroll
-        for (int c = 0; c < NC; ++c) acc[r][c] += (double)pa[r][c];
-        acc[r][NC - 1] = -acc[r][NC - 1];  // pot = - Sum m/r
-    }
+    flush(pa, acc_mine);
+    __syncthreads();
 
-    // ---- epilogue ----
-    auto store = [&](int comp, int slot, double val) {
-        if (A.splits == 1) {
-            if (comp == NC - 1) A.out[4][slot] = val;
-            else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = val;
-        } else {
-            A.partials[((size_t)blockIdx.y * NC + comp) * A.n_act + slot] = val;
-        }
-    };
-    if (JL == 1) {
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int slot = blockIdx.x * (IT * R) + r * IT + il;
-            if (slot < A.n_act) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) store(c, slot, acc[r][c]);
+    // ---- epilogue: fixed-order sum over the JL j-lanes, pot = - Sum m/r ----
+    for (int o = tid; o < 2 * IT * NC; o += kThreads) {
+        const int comp = o / (2 * IT), rem = o % (2 * IT);
+        const int r = rem / IT, i_l = rem % IT;
+        double sum = 0.0;
+#pragma unroll 1
+        for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
+        const int slot = blockIdx.x * (2 * IT) + r * IT + i_l;
+        if (slot < A.n_act) {
+            if (comp == NC - 1) sum = -sum;
+            if (A.splits == 1) {
+                if (comp == NC - 1) A.out[4][slot] = sum;
+                else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
+            } else {
+                A.partials[((size_t)blockIdx.y * NC + comp) * A.n_act + slot] = sum;
             }
-        }
-    } else {
-        __syncthreads();  // tiles are dead: reuse them as the reduction buffer red[jl][comp][il]
-        double *red = reinterpret_cast<double *>(smem_raw);
-#pragma unroll
-        for (int c = 0; c < NC; ++c) red[(jl * NC + c) * IT + il] = acc[0][c];
-        __syncthreads();
-        for (int o = tid; o < IT * NC; o += kThreads) {
-            const int comp = o / IT, i_l = o % IT;
-            double sum = 0.0;
-            for (int l = 0; l < JL; ++l) sum += red[(l * NC + comp) * IT + i_l];
-            const int slot = blockIdx.x * IT + i_l;
-            if (slot < A.n_act) store(comp, slot, sum);
         }
     }
 }
@@ -363,51 +435,47 @@ __global__ void __launch_bounds__(256) k_reduce(const double *partials, int spli
     }
 }
 
-template <int ORDER>
-constexpr size_t force_smem() {
-    return (size_t)kStages * (ORDER == 4 ? 3 : 4) * kTileJ * 16 + 8 * kStages + 64;
-}
-
 typedef void (*force_fn)(const ForceArgs);
 
 template <int ORDER, int DIFF>
-force_fn pick(int r, int jl) {
-    if (r == 2) return k_force<ORDER, 2, 1, DIFF>;
+force_fn pick(int jl) {
     switch (jl) {
-        case 1: return k_force<ORDER, 1, 1, DIFF>;
-        case 4: return k_force<ORDER, 1, 4, DIFF>;
-        case 16: return k_force<ORDER, 1, 16, DIFF>;
-        case 64: return k_force<ORDER, 1, 64, DIFF>;
-        default: return k_force<ORDER, 1, 256, DIFF>;
+        case 1: return k_force<ORDER, 1, DIFF>;
+        case 4: return k_force<ORDER, 4, DIFF>;
+        case 16: return k_force<ORDER, 16, DIFF>;
+        case 64: return k_force<ORDER, 64, DIFF>;
+        default: return k_force<ORDER, 128, DIFF>;
     }
 }
 
-force_fn pick_fn(int order, int diff, int r, int jl) {
+force_fn pick_fn(int order, int diff, int jl) {
     if (diff == 0) {
-        if (order == 4) return pick<4, 0>(r, jl);
-        if (order == 6) return pick<6, 0>(r, jl);
-        return pick<8, 0>(r, jl);
+        if (order == 4) return pick<4, 0>(jl);
+        if (order == 6) return pick<6, 0>(jl);
+        return pick<8, 0>(jl);
     }
-    if (order == 4) return pick<4, 1>(r, jl);
-    if (order == 6) return pick<6, 1>(r, jl);
-    return pick<8, 1>(r, jl);
+    if (order == 4) return pick<4, 1>(jl);
+    if (order == 6) return pick<6, 1>(jl);
+    return pick<8, 1>(jl);
 }
 
-size_t smem_for(int order) { return order == 4 ? force_smem<4>() : force_smem<6>(); }
+size_t smem_for(int order, int diff) {
+    if (diff == 0) return order == 4 ? Geo<4, 0>::SMEM : order == 6 ? Geo<6, 0>::SMEM : Geo<8, 0>::SMEM;
+    return order == 4 ? Geo<4, 1>::SMEM : order == 6 ? Geo<6, 1>::SMEM : Geo<8, 1>::SMEM;
+}
+
+const int kLanes[5] = {1, 4, 16, 64, 128};
 
 }  // namespace
 
 int force_static_init(Ctx *c) {
     const int orders[3] = {4, 6, 8};
-    const int jls[5] = {1, 4, 16, 64, 256};
     for (int diff = 0; diff < 2; ++diff)
-        for (int o = 0; o < 3; ++o) {
-            NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, 2, 1),
-                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(orders[o])));
+        for (int o = 0; o < 3; ++o)
             for (int j = 0; j < 5; ++j)
-                NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, 1, jls[j]),
-                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(orders[o])));
-        }
+                NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, kLanes[j]),
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)smem_for(orders[o], diff)));
     return NBODY_OK;
 }
 
@@ -415,19 +483,11 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
                  double *snap, double *crackle, double *pot, cudaStream_t st) {
     const int K = order / 2, NC = 3 * K + 1;
     const int n_tiles = (int)(c->n_pad / kTileJ);
-    // geometry: i per thread, j-lanes, i-tiles, j-splits
-    int r, jl;
-    if (c->force_lanes) {
-        r = 1;
-        jl = c->force_lanes;
-    } else if (n_act > 256) {
-        r = 2;
-        jl = 1;
-    } else {
-        r = 1;
-        jl = n_act > 64 ? 1 : n_act > 16 ? 4 : n_act > 4 ? 16 : n_act > 1 ? 64 : 256;
-    }
-    const int i_per_cta = (kThreads / jl) * r;
+    // geometry: j-lanes (a CTA owns 2 * 256 / JL i-particles), i-tiles, j-splits
+    int jl;
+    if (c->force_lanes) jl = c->force_lanes;
+    else jl = n_act > 128 ? 1 : n_act > 32 ? 4 : n_act > 8 ? 16 : n_act > 4 ? 64 : 128;
+    const int i_per_cta = 2 * (kThreads / jl);
     const int64_t i_tiles = (n_act + i_per_cta - 1) / i_per_cta;
     const int64_t target = 2 * (int64_t)c->sm_count;  // 2 resident CTAs per SM
     int64_t S = c->force_split ? c->force_split : (i_tiles >= target ? 1 : (target + i_tiles - 1) / i_tiles);
@@ -447,10 +507,14 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     }
     ForceArgs A;
     const uint4 *base = c->jstore;
-    A.q[0] = base + (size_t)(c->diff_mode ? 4 : 0) * c->cap_pad;
-    A.q[1] = base + (size_t)(c->diff_mode ? 5 : 1) * c->cap_pad;
-    A.q[2] = base + (size_t)2 * c->cap_pad;
-    A.q[3] = base + (size_t)3 * c->cap_pad;
+    int np = 0;
+    if (c->diff_mode) {
+        for (int p = 0; p < 3; ++p) A.q[np++] = base + (size_t)(kPlaneD0 + p) * c->cap_pad;
+    } else {
+        A.q[np++] = base;
+    }
+    for (int p = 1; p <= 6; ++p) A.q[np++] = base + (size_t)p * c->cap_pad;
+    for (; np < 9; ++np) A.q[np] = nullptr;
     A.idx = active_idx;
     A.n_act = (int)n_act;
     A.n_tiles = n_tiles;
@@ -459,7 +523,7 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     A.out[0] = acc; A.out[1] = jerk; A.out[2] = snap; A.out[3] = crackle; A.out[4] = pot;
     A.partials = c->partials;
     const dim3 grid((unsigned)i_tiles, (unsigned)S);
-    pick_fn(order, c->diff_mode, r, jl)<<<grid, kThreads, smem_for(order), st>>>(A);
+    pick_fn(order, c->diff_mode, jl)<<<grid, kThreads, smem_for(order, c->diff_mode), st>>>(A);
     c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
     if (S > 1) {
@@ -469,7 +533,7 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
         c->launches += 1;
         NB_CUDA(c, cudaGetLastError());
     }
-    c->last_r = r;
+    c->last_r = 2;
     c->last_jl = jl;
     c->last_s = (int)S;
     c->last_ctas = i_tiles * S;

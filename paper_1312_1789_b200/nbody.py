@@ -9,7 +9,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "csrc", "libnbody.so")
+LIB_PATH = os.environ.get("NBODY_LIBRARY") or os.path.join(_HERE, "csrc", "libnbody.so")  # override: another build
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
