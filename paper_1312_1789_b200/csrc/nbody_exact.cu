@@ -103,48 +103,46 @@ __global__ void __launch_bounds__(256) k_predict(PredArgs A) {
         vp[0] = vp[1] = vp[2] = 0.f;
     }
     A.q[0][i] = pack_dd(xp[0], xp[1]);
-    A.q[1][i] = pack_dff(xp[2], m32, m32);
-    A.q[2][i] = pack_ffff(vp[0], vp[0], vp[1], vp[1]);
-    A.q[3][i] = pack_ffff(vp[2], vp[2], ap[0], ap[0]);
-    if (ORDER >= 6) A.q[4][i] = pack_ffff(ap[1], ap[1], ap[2], ap[2]);
-    if (ORDER >= 8) {
-        A.q[5][i] = pack_ffff(jp[0], jp[0], jp[1], jp[1]);
-        A.q[6][i] = pack_ffff(jp[2], jp[2], 0.f, 0.f);
-    }
+    A.q[1][i] = pack_dff(xp[2], m32, vp[0]);
+    A.q[2][i] = pack_ffff(vp[1], vp[2], ap[0], ap[1]);
+    if (ORDER >= 6) A.q[3][i] = pack_ffff(ap[2], jp[0], jp[1], jp[2]);
     if (A.write_ds) {
+        float hi[3], lo[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const float hi = __double2float_rn(xp[d]);
-            const float lo = __double2float_rn(dsub(xp[d], (double)hi));
-            A.q[kPlaneD0 + d][i] = pack_ffff(hi, hi, lo, lo);
+            hi[d] = __double2float_rn(xp[d]);
+            lo[d] = __double2float_rn(dsub(xp[d], (double)hi[d]));
         }
+        A.q[4][i] = pack_ffff(hi[0], lo[0], hi[1], lo[1]);
+        A.q[5][i] = pack_ffff(hi[2], lo[2], m32, vp[0]);
     }
 }
 
 // export of the j-store (test hook)
-__global__ void k_unpack(const uint4 *jstore, long long cap_pad, long long n, int order, double *xp, float *vp,
-                         float *ap, float *jp, float *m32) {
+__global__ void k_unpack(const uint4 *q0, const uint4 *q1, const uint4 *q2, const uint4 *q3, long long n, int order,
+                         double *xp, float *vp, float *ap, float *jp, float *m32) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const uint4 a = jstore[i], b = jstore[cap_pad + i], c = jstore[2 * cap_pad + i], d = jstore[3 * cap_pad + i];
+    const uint4 a = q0[i], b = q1[i], c = q2[i];
     xp[3 * i + 0] = __longlong_as_double(((long long)a.y << 32) | a.x);
     xp[3 * i + 1] = __longlong_as_double(((long long)a.w << 32) | a.z);
     xp[3 * i + 2] = __longlong_as_double(((long long)b.y << 32) | b.x);
     m32[i] = __uint_as_float(b.z);
-    vp[3 * i + 0] = __uint_as_float(c.x);
-    vp[3 * i + 1] = __uint_as_float(c.z);
-    vp[3 * i + 2] = __uint_as_float(d.x);
-    if (order >= 6 && ap) {
-        const uint4 e = jstore[4 * cap_pad + i];
-        ap[3 * i + 0] = __uint_as_float(d.z);
-        ap[3 * i + 1] = __uint_as_float(e.x);
-        ap[3 * i + 2] = __uint_as_float(e.z);
-    }
-    if (order >= 8 && jp) {
-        const uint4 f = jstore[5 * cap_pad + i], g = jstore[6 * cap_pad + i];
-        jp[3 * i + 0] = __uint_as_float(f.x);
-        jp[3 * i + 1] = __uint_as_float(f.z);
-        jp[3 * i + 2] = __uint_as_float(g.x);
+    vp[3 * i + 0] = __uint_as_float(b.w);
+    vp[3 * i + 1] = __uint_as_float(c.x);
+    vp[3 * i + 2] = __uint_as_float(c.y);
+    if (order >= 6) {
+        const uint4 d = q3[i];
+        if (ap) {
+            ap[3 * i + 0] = __uint_as_float(c.z);
+            ap[3 * i + 1] = __uint_as_float(c.w);
+            ap[3 * i + 2] = __uint_as_float(d.x);
+        }
+        if (jp && order >= 8) {
+            jp[3 * i + 0] = __uint_as_float(d.y);
+            jp[3 * i + 1] = __uint_as_float(d.z);
+            jp[3 * i + 2] = __uint_as_float(d.w);
+        }
     }
 }
 
@@ -667,8 +665,9 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
     if (c->n < 0) return NBODY_ESTATE;
     if ((ap && c->pred_order < 6) || (jp && c->pred_order < 8)) return NBODY_EINVAL;
     if (c->n == 0) return NBODY_OK;
-    k_unpack<<<(unsigned)((c->n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c->jstore, c->cap_pad, c->n, c->pred_order,
-                                                                                xp, vp, ap, jp, m32);
+    const uint4 *q = c->jstore;
+    k_unpack<<<(unsigned)((c->n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        q, q + c->cap_pad, q + 2 * c->cap_pad, q + 3 * c->cap_pad, c->n, c->pred_order, xp, vp, ap, jp, m32);
     c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
     return NBODY_OK;

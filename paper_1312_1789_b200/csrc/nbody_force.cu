@@ -7,7 +7,7 @@
 //     The scalar form is limited by issue slots and by register-file bandwidth (a 3-source FFMA with two sources in
 //     the same register bank takes 2 cycles); the packed form reads aligned 64-bit register pairs and halves the
 //     instruction count of the fp32 part.  The j operand of a packed instruction is the broadcast pair {v, v},
-//     which is why the j-store keeps fp32 values twice (nbody_internal.h);
+//     which ptxas folds into a 32-bit broadcast register operand (SASS `Rn.F32`), so the j-store stays compact;
 //   - j-tiles of kTileJ particles are staged plane by plane into shared memory by 1-D TMA bulk copies
 //     (cp.async.bulk + mbarrier) through a ring; every pair-loop read is an LDS.128 broadcast;
 //   - d = fl32(x_j - x_i) with the subtraction in fp64 (DIFF 0: DADD + F2F per lane) or double-single (DIFF 1:
@@ -88,6 +88,8 @@ __device__ __forceinline__ f2 pku(unsigned a, unsigned b) {
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(a), "r"(b));
     return r;
 }
+// broadcast pair {v, v}: ptxas folds it into a 32-bit broadcast operand (Rn.F32) of the packed instruction
+__device__ __forceinline__ f2 bc(unsigned v) { return pku(v, v); }
 __device__ __forceinline__ void upk(f2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ f2 add2(f2 a, f2 b) {
     f2 r;
@@ -109,9 +111,8 @@ template <int ORDER, int DIFF>
 struct Geo {
     static constexpr int K = ORDER / 2;
     static constexpr int NC = 3 * K + 1;                        // components per i: 3K vectors + pot
-    static constexpr int XP = DIFF ? 3 : 1;                     // position planes (P0 | D0, D1, D2)
-    static constexpr int NQ = XP + (ORDER == 4 ? 3 : ORDER == 6 ? 4 : 6);  // planes staged per tile
-    static constexpr int STAGES = NQ >= 7 ? 3 : 4;              // TMA ring depth
+    static constexpr int NQ = ORDER == 4 ? 3 : 4;               // planes staged per tile (Q0..Q3 | Q4, Q5, Q2, Q3)
+    static constexpr int STAGES = 4;                            // TMA ring depth
     static constexpr uint32_t STAGE_BYTES = NQ * kTileJ * 16;
     static constexpr size_t TILE_BYTES = (size_t)STAGES * STAGE_BYTES;
     static constexpr size_t ACC_BYTES = (size_t)2 * NC * kThreads * sizeof(double);
@@ -119,7 +120,7 @@ struct Geo {
 };
 
 struct ForceArgs {
-    const uint4 *q[9];  // planes in kernel order: position planes, then P1, P2, ...
+    const uint4 *q[4];  // planes in use: {Q0,Q1,Q2,Q3} (DIFF 0) or {Q4,Q5,Q2,Q3} (DIFF 1)
     const int32_t *idx;
     int n_act;
     int n_tiles;
@@ -146,30 +147,25 @@ struct Consts {  // loop-invariant packed constants
 template <int ORDER, int DIFF, bool MASK>
 __device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *tq, int jt, int jglob,
                                       const Consts &C, f2 *pa) {
-    typedef Geo<ORDER, DIFF> G;
-    constexpr int XP = G::XP;
     f2 d[3];
-    const uint4 qb = tq[XP * kTileJ + jt];  // P1 = { z (f64), m, m }
+    const uint4 qa = tq[jt];           // Q0 = { x, y } (f64)           | Q4 = { xhi, xlo, yhi, ylo }
+    const uint4 qb = tq[kTileJ + jt];  // Q1 = { z (f64), m, vx }       | Q5 = { zhi, zlo, m, vx }
     if (DIFF == 0) {
-        const uint4 qa = tq[jt];  // P0 = { x, y }
         const double xj = u2d(qa.x, qa.y), yj = u2d(qa.z, qa.w), zj = u2d(qb.x, qb.y);
         d[0] = pk(d2f(xj - I.x[0][0]), d2f(xj - I.x[1][0]));
         d[1] = pk(d2f(yj - I.x[0][1]), d2f(yj - I.x[1][1]));
         d[2] = pk(d2f(zj - I.x[0][2]), d2f(zj - I.x[1][2]));
     } else {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const uint4 qx = tq[c * kTileJ + jt];  // Dc = { hi, hi, lo, lo }
-            d[c] = add2(add2(pku(qx.x, qx.y), I.nxh[c]), add2(pku(qx.z, qx.w), I.nxl[c]));
-        }
+        d[0] = add2(add2(bc(qa.x), I.nxh[0]), add2(bc(qa.y), I.nxl[0]));
+        d[1] = add2(add2(bc(qa.z), I.nxh[1]), add2(bc(qa.w), I.nxl[1]));
+        d[2] = add2(add2(bc(qb.x), I.nxh[2]), add2(bc(qb.y), I.nxl[2]));
     }
-    const f2 mj = pku(qb.z, qb.w);
-    const uint4 qc = tq[(XP + 1) * kTileJ + jt];  // P2 = { vx, vx, vy, vy }
-    const uint4 qd = tq[(XP + 2) * kTileJ + jt];  // P3 = { vz, vz, ax, ax }
+    const f2 mj = bc(qb.z);
+    const uint4 qc = tq[2 * kTileJ + jt];  // Q2 = { vy, vz, ax, ay }
     f2 dv[3], da[3], dj[3];
-    dv[0] = add2(pku(qc.x, qc.y), I.nv[0]);
-    dv[1] = add2(pku(qc.z, qc.w), I.nv[1]);
-    dv[2] = add2(pku(qd.x, qd.y), I.nv[2]);
+    dv[0] = add2(bc(qb.w), I.nv[0]);
+    dv[1] = add2(bc(qc.x), I.nv[1]);
+    dv[2] = add2(bc(qc.y), I.nv[2]);
     f2 r2 = fma2(d[0], d[0], C.eps2);
     r2 = fma2(d[1], d[1], r2);
     r2 = fma2(d[2], d[2], r2);
@@ -200,10 +196,10 @@ __device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *
         pa[3 + c] = fma2(q, Jp[c], pa[3 + c]);
     }
     if (ORDER >= 6) {
-        const uint4 qe = tq[(XP + 3) * kTileJ + jt];  // P4 = { ay, ay, az, az }
-        da[0] = add2(pku(qd.z, qd.w), I.na[0]);
-        da[1] = add2(pku(qe.x, qe.y), I.na[1]);
-        da[2] = add2(pku(qe.z, qe.w), I.na[2]);
+        const uint4 qd = tq[3 * kTileJ + jt];  // Q3 = { az, jx, jy, jz }
+        da[0] = add2(bc(qc.z), I.na[0]);
+        da[1] = add2(bc(qc.w), I.na[1]);
+        da[2] = add2(bc(qd.x), I.na[2]);
         f2 w = mul2(dv[0], dv[0]);
         w = fma2(dv[1], dv[1], w);
         w = fma2(dv[2], dv[2], w);
@@ -220,11 +216,9 @@ __device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *
             pa[6 + c] = fma2(q, Sp[c], pa[6 + c]);
         }
         if (ORDER >= 8) {
-            const uint4 qf = tq[(XP + 4) * kTileJ + jt];  // P5 = { jx, jx, jy, jy }
-            const uint4 qg = tq[(XP + 5) * kTileJ + jt];  // P6 = { jz, jz, 0, 0 }
-            dj[0] = add2(pku(qf.x, qf.y), I.nj[0]);
-            dj[1] = add2(pku(qf.z, qf.w), I.nj[1]);
-            dj[2] = add2(pku(qg.x, qg.y), I.nj[2]);
+            dj[0] = add2(bc(qd.y), I.nj[0]);
+            dj[1] = add2(bc(qd.z), I.nj[1]);
+            dj[2] = add2(bc(qd.w), I.nj[2]);
             f2 va = mul2(dv[0], da[0]);
             va = fma2(dv[1], da[1], va);
             va = fma2(dv[2], da[2], va);
@@ -279,7 +273,7 @@ __device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const 
 template <int ORDER, int JL, int DIFF>
 __global__ void __launch_bounds__(kThreads, 2) k_force(const ForceArgs A) {
     typedef Geo<ORDER, DIFF> G;
-    constexpr int NQ = G::NQ, NC = G::NC, XP = G::XP, STAGES = G::STAGES;
+    constexpr int NQ = G::NQ, NC = G::NC, STAGES = G::STAGES;
     constexpr int IT = kThreads / JL;    // threads per j-lane; the CTA owns 2 IT i-particles
     constexpr int JPT = kTileJ / JL;     // j-particles per thread and tile
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -320,34 +314,27 @@ __global__ void __launch_bounds__(kThreads, 2) k_force(const ForceArgs A) {
         const bool valid = slot < A.n_act;
         const int gi = A.idx[valid ? slot : A.n_act - 1];
         I.idx[r] = valid ? gi : -1;
-        const uint4 qb = __ldg(A.q[XP] + gi), qc = __ldg(A.q[XP + 1] + gi), qd = __ldg(A.q[XP + 2] + gi);
+        const uint4 qa = __ldg(A.q[0] + gi), qb = __ldg(A.q[1] + gi), qc = __ldg(A.q[2] + gi);
         if (DIFF == 0) {
-            const uint4 qa = __ldg(A.q[0] + gi);
             I.x[r][0] = u2d(qa.x, qa.y);
             I.x[r][1] = u2d(qa.z, qa.w);
             I.x[r][2] = u2d(qb.x, qb.y);
         } else {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const uint4 qx = __ldg(A.q[c] + gi);
-                xh[r][c] = -u2f(qx.x);
-                xl[r][c] = -u2f(qx.z);
-            }
+            xh[r][0] = -u2f(qa.x); xl[r][0] = -u2f(qa.y);
+            xh[r][1] = -u2f(qa.z); xl[r][1] = -u2f(qa.w);
+            xh[r][2] = -u2f(qb.x); xl[r][2] = -u2f(qb.y);
         }
-        nv[r][0] = -u2f(qc.x);
-        nv[r][1] = -u2f(qc.z);
-        nv[r][2] = -u2f(qd.x);
+        nv[r][0] = -u2f(qb.w);
+        nv[r][1] = -u2f(qc.x);
+        nv[r][2] = -u2f(qc.y);
         if (ORDER >= 6) {
-            const uint4 qe = __ldg(A.q[XP + 3] + gi);
-            na[r][0] = -u2f(qd.z);
-            na[r][1] = -u2f(qe.x);
-            na[r][2] = -u2f(qe.z);
-        }
-        if (ORDER >= 8) {
-            const uint4 qf = __ldg(A.q[XP + 4] + gi), qg = __ldg(A.q[XP + 5] + gi);
-            nj[r][0] = -u2f(qf.x);
-            nj[r][1] = -u2f(qf.z);
-            nj[r][2] = -u2f(qg.x);
+            const uint4 qd = __ldg(A.q[3] + gi);
+            na[r][0] = -u2f(qc.z);
+            na[r][1] = -u2f(qc.w);
+            na[r][2] = -u2f(qd.x);
+            nj[r][0] = -u2f(qd.y);
+            nj[r][1] = -u2f(qd.z);
+            nj[r][2] = -u2f(qd.w);
         }
     }
 #pragma unroll
@@ -507,14 +494,10 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     }
     ForceArgs A;
     const uint4 *base = c->jstore;
-    int np = 0;
-    if (c->diff_mode) {
-        for (int p = 0; p < 3; ++p) A.q[np++] = base + (size_t)(kPlaneD0 + p) * c->cap_pad;
-    } else {
-        A.q[np++] = base;
-    }
-    for (int p = 1; p <= 6; ++p) A.q[np++] = base + (size_t)p * c->cap_pad;
-    for (; np < 9; ++np) A.q[np] = nullptr;
+    A.q[0] = base + (size_t)(c->diff_mode ? 4 : 0) * c->cap_pad;
+    A.q[1] = base + (size_t)(c->diff_mode ? 5 : 1) * c->cap_pad;
+    A.q[2] = base + (size_t)2 * c->cap_pad;
+    A.q[3] = base + (size_t)3 * c->cap_pad;
     A.idx = active_idx;
     A.n_act = (int)n_act;
     A.n_tiles = n_tiles;

@@ -9,16 +9,13 @@
 namespace nbody {
 
 // ---- packed j-store ---------------------------------------------------------------
-// Planes of 16-byte quads, plane p at jstore + p * cap_pad (in quads).  fp32 values are stored TWICE so that one
-// 64-bit half of a quad is the broadcast operand {v, v} of a packed f32x2 instruction (two i-particles per thread):
-//   P0 = { x (f64), y (f64) }            P1 = { z (f64), m, m }
-//   P2 = { vx, vx, vy, vy }              P3 = { vz, vz, ax, ax }
-//   P4 = { ay, ay, az, az }              P5 = { jx, jx, jy, jy }            P6 = { jz, jz, 0, 0 }
-//   D0 = { xhi, xhi, xlo, xlo }          D1 = { yhi, yhi, ylo, ylo }        D2 = { zhi, zhi, zlo, zlo }
-// order 4 reads P0..P3, order 6 P0..P4, order 8 P0..P6; diff_mode 1 (double-single) reads D0..D2 instead of P0.
-// Entries [n, n_pad) are zero-mass pads parked far away.
-constexpr int kPlanes = 10;
-constexpr int kPlaneD0 = 7;
+// Planes of 16-byte quads, plane p at jstore + p * cap_pad (in quads):
+//   Q0 = { x (f64), y (f64) }            Q1 = { z (f64), m (f32), vx (f32) }
+//   Q2 = { vy, vz, ax, ay } (f32)        Q3 = { az, jx, jy, jz } (f32)
+//   Q4 = { xhi, xlo, yhi, ylo } (f32)    Q5 = { zhi, zlo, m, vx } (f32)     (double-single twin of Q0/Q1)
+// order 4 reads Q0..Q2, order 6 and 8 read Q0..Q3; diff_mode 1 reads Q4, Q5 instead of Q0, Q1.  The force kernel
+// feeds a j-value to both lanes of a packed f32x2 instruction as a broadcast 32-bit register operand.  Entries [n, n_pad) are zero-mass pads parked far away.
+constexpr int kPlanes = 6;
 constexpr int kTileJ = 128;    // j-particles per TMA stage (and the padding granule of the j-store)
 constexpr int kThreads = 256;  // threads per force CTA
 constexpr double kPadPos = 1.0e6;
