@@ -44,7 +44,7 @@ def parse():
     ap.add_argument("--n", type=int, default=1048576)
     ap.add_argument("--order", type=int, default=6, choices=[4, 6, 8])
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--cpu-sample", type=int, default=1536, help="i-particles of the cpu_baseline leg")
+    ap.add_argument("--cpu-sample", type=int, default=12288, help="i-particles of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -330,6 +330,10 @@ def main():
         torch.cuda.synchronize()
         keep_state = {"t": g.t.cpu().numpy().copy(), "dt": g.dt.cpu().numpy().copy(),
                       "D": [d.cpu().numpy().copy() for d in g.D[:order - 2]]}
+        # instruction-class micro-probes (1e12 thread-ops/s, SM MHz inside the probe): context for the roofline
+        names = {0: "ffma", 5: "ffma2_two_fresh_operands", 6: "ffma2_three_fresh_operands", 1: "dadd",
+                 2: "f2f_f64_f32_roundtrip", 3: "mufu_rsq"}
+        line["probes_tera_ops"] = {nm: [round(v, 3) for v in g.ctx.probe_peak(k, 150)] for k, nm in names.items()}
         if not args.no_e2e:
             line["e2e"] = e2e_leg(args, g, c, order, eps2, H)
         if not args.no_cpu_baseline and world == 1:

@@ -178,7 +178,8 @@ int nbody_step_host(nbody_ctx *ctx, int64_t n, int order, double eps2, double et
  * rate in 1e12 thread-operations per second in tera_ops_host[0] (an FFMA counts as ONE operation) and the SM
  * clock in MHz measured inside that kernel (clock64 / globaltimer) in tera_ops_host[1]; HOST array of 2.
  *   kind 0 = FFMA (fp32), 1 = DADD (fp64 add), 2 = F2F (fp64->fp32->fp64 round trip, 2 ops), 3 = MUFU.RSQ,
- *   4 = the literal difference pattern DADD + F2F + FADD (3 ops).
+ *   4 = the literal difference pattern DADD + F2F + FADD (3 ops), 5 = packed FFMA2 with two fresh 64-bit register
+ *   operands, 6 = packed FFMA2 with three fresh operands (one FFMA2 = ONE operation = 4 flops).
  * Synchronises.
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_probe_peak(nbody_ctx *ctx, int kind, int millis, double *tera_ops_host);

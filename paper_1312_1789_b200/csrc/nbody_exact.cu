@@ -674,7 +674,7 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
 }
 
 int nbody_probe_peak(nbody_ctx *h, int kind, int millis, double *tera_ops_host) {
-    if (!h || !tera_ops_host || kind < 0 || kind > 4 || millis < 1 || millis > 20000) return NBODY_EINVAL;
+    if (!h || !tera_ops_host || kind < 0 || kind > 6 || millis < 1 || millis > 20000) return NBODY_EINVAL;
     return probe_peak(&h->c, kind, millis, tera_ops_host);
 }
 

@@ -23,7 +23,7 @@
 #include "nbody_internal.h"
 
 #ifndef NB_UNROLL
-#define NB_UNROLL 2
+#define NB_UNROLL 4
 #endif
 
 namespace nbody {
@@ -162,10 +162,11 @@ __device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *
     }
     const f2 mj = bc(qb.z);
     const uint4 qc = tq[2 * kTileJ + jt];  // Q2 = { vy, vz, ax, ay }
-    f2 dv[3], da[3], dj[3];
+    f2 dv[3], dj[3];
     dv[0] = add2(bc(qb.w), I.nv[0]);
     dv[1] = add2(bc(qc.x), I.nv[1]);
     dv[2] = add2(bc(qc.y), I.nv[2]);
+    f2 da[3];
     f2 r2 = fma2(d[0], d[0], C.eps2);
     r2 = fma2(d[1], d[1], r2);
     r2 = fma2(d[2], d[2], r2);

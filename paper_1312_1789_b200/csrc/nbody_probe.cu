@@ -23,6 +23,14 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
         f[c] = seed + (float)(threadIdx.x + c);
         d[c] = (double)seed + (double)(threadIdx.x * 3 + c);
     }
+    unsigned long long p2[kProbeChains], p2c[kProbeChains], p2d[kProbeChains], p2b;
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) {
+        asm("mov.b64 %0, {%1, %2};" : "=l"(p2[c]) : "f"(seed + c), "f"(seed - c));
+        asm("mov.b64 %0, {%1, %2};" : "=l"(p2c[c]) : "f"(1e-3f * c + seed), "f"(2e-3f));
+        asm("mov.b64 %0, {%1, %2};" : "=l"(p2d[c]) : "f"(0.999f + seed * c), "f"(0.998f + seed * c));
+    }
+    asm("mov.b64 %0, {%1, %2};" : "=l"(p2b) : "f"(0.999f + seed), "f"(0.998f + seed));
     const float b = 0.999f + seed, cc = 1e-3f;
     const double db = 1e-3 + (double)seed;
 #pragma unroll 8
@@ -36,6 +44,10 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
                 asm volatile("cvt.f64.f32 %0, %1;" : "=d"(d[c]) : "f"(f[c]));
             }
             if (KIND == 3) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f[c]));
+            if (KIND == 5)  // packed FFMA2, two fresh 64-bit operands (one shared): the pair loop's common form
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p2[c]) : "l"(p2b), "l"(p2c[c]));
+            if (KIND == 6)  // packed FFMA2, three fresh 64-bit operands
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p2[c]) : "l"(p2d[c]), "l"(p2c[c]));
             if (KIND == 4) {  // the literal difference pattern: DADD, F2F, and an FADD that consumes it
                 double t;
                 float g;
@@ -48,7 +60,13 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
     }
     float s = 0.f;
 #pragma unroll
-    for (int c = 0; c < kProbeChains; ++c) s += f[c] + (float)d[c];
+    for (int c = 0; c < kProbeChains; ++c) {
+        float lo, hi, lo2, hi2, lo3, hi3;
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p2[c]));
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo2), "=f"(hi2) : "l"(p2c[c]));
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo3), "=f"(hi3) : "l"(p2d[c]));
+        s += f[c] + (float)d[c] + lo + hi + lo2 + hi2 + lo3 + hi3;
+    }
     if (s == 123.456f) sink[0] = s;  // never true in practice; keeps the chains live
     if (blockIdx.x == 0 && threadIdx.x == 0) {  // SM cycles and nanoseconds this CTA ran: the SM clock under this load
         unsigned long long g1;
@@ -60,7 +78,7 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
 }
 
 typedef void (*probe_fn)(float *, float, unsigned long long *);
-const probe_fn kProbes[5] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>};
+const probe_fn kProbes[7] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>, k_probe<5>, k_probe<6>};
 
 }  // namespace
 
