@@ -1,0 +1,82 @@
+"""-m gpu: parity at BASELINE.json's FULL sizes, in the launch configurations bench.py times, on sampled outputs the
+oracle computes one by one (forced members: every BH, innermost / outermost particles, nearest to each BH, plus a
+seeded draw -- where mixed-precision errors are largest).
+
+  config 4: N = 1 048 576, 6th order, ALL active (the bench.py launch: 2048 CTAs, no j-split)
+  config 3: N =   262 144, 6th order, N_act sweep 4^0 .. 4^9 (every lane variant and j-split at full N)
+  config 2: N =    65 536, 4th order, N_act = 1, 16, 256, 4096, 65 536
+  config 5: N = 2 097 152, 8th order, ALL active
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_1312_1789_b200 import workloads as W
+import gpu_util as U
+
+
+def _setup(config, order):
+    import torch
+    from paper_1312_1789_b200 import nbody
+    c = W.cluster(config)
+    n = c["n"]
+    D = W.smooth_field_derivs(c, 6)
+    t, dt = W.predictor_times(c["x"])
+    t_now = 2.0**-10
+    ctx = nbody.Context(n)
+    ctx.predict(n, t_now, order, U.dev(t), U.dev(c["m"]), U.dev(c["x"]), U.dev(c["v"]), [U.dev(d) for d in D[: order - 2]])
+    from oracle import oracle as O
+    xp, vp, ap, jp = O.predict(t_now, order, t, c["x"], c["v"], D)
+    return c, n, ctx, O, (xp, vp, ap, jp)
+
+
+def _force(ctx, idx_dev, n_act, order, eps2):
+    import torch
+    acc, jerk, pot = U.zeros(n_act, 3), U.zeros(n_act, 3), U.zeros(n_act)
+    snap = U.zeros(n_act, 3) if order >= 6 else None
+    crk = U.zeros(n_act, 3) if order >= 8 else None
+    ctx.force(idx_dev, n_act, order, eps2, acc, jerk, snap, crk, pot)
+    torch.cuda.synchronize()
+    return acc, jerk, snap, crk, pot
+
+
+@pytest.mark.parametrize("config,order,sample", [(4, 6, 1024), (5, 8, 512)])
+def test_all_active_full_size_sampled(config, order, sample):
+    import torch
+    c, n, ctx, O, (xp, vp, ap, jp) = _setup(config, order)
+    idx_all = torch.arange(n, dtype=torch.int32, device="cuda")
+    out = _force(ctx, idx_all, n, order, c["eps2"])
+    g = ctx.last_force_geometry()
+    assert g["j_lanes"] == 1 and g["j_splits"] == 1 and g["ctas"] == (n + 511) // 512  # the configuration bench.py times
+    s = W.oracle_sample(c, size=sample)
+    ref = O.force(c["m"], xp, vp, ap, jp, s, order, c["eps2"])
+    ii = torch.from_numpy(s.astype(np.int64)).cuda()
+    got = tuple(None if a is None else a[ii].cpu().numpy() for a in out)
+    errs = U.check_force(got, ref, order, "cfg%d all-active N=%d" % (config, n))
+    print("cfg%d N=%d order %d sampled max rel errors: %s" % (config, n, order, errs))
+    ctx.close()
+
+
+@pytest.mark.parametrize("config,order,nacts", [(3, 6, [4**k for k in range(10)]), (2, 4, [1, 16, 256, 4096, 65536])])
+def test_nact_sweep_full_size_sampled(config, order, nacts):
+    import torch
+    c, n, ctx, O, (xp, vp, ap, jp) = _setup(config, order)
+    rng = W.rng_for(config, 31)
+    forced = W.oracle_sample(c, size=160)  # forced members only (+ a few): always part of every active list
+    for n_act in nacts:
+        n_act = min(n_act, n)
+        idx = W.active_list(n, n_act, rng)
+        if n_act < n:
+            k = min(forced.shape[0], n_act)
+            idx = np.unique(np.concatenate([idx[: n_act - k], forced[:k]])).astype(np.int32)
+        na = idx.shape[0]
+        out = _force(ctx, U.dev(idx), na, order, c["eps2"])
+        # oracle on <= 1024 of the active particles (positions inside the active list)
+        pick = np.arange(na) if na <= 1024 else np.unique(np.concatenate(
+            [np.nonzero(np.isin(idx, forced))[0], rng.choice(na, 1024 - forced.shape[0], replace=False)]))
+        ref = O.force(c["m"], xp, vp, ap, jp, idx[pick], order, c["eps2"])
+        pp = torch.from_numpy(pick.astype(np.int64)).cuda()
+        got = tuple(None if a is None else a[pp].cpu().numpy() for a in out)
+        U.check_force(got, ref, order, "cfg%d N=%d n_act=%d geom %s" % (config, n, na, ctx.last_force_geometry()))
+    ctx.close()
