@@ -62,7 +62,7 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 dt = eta (A^(1)/A^(pc-2))^(1/(pc-3)) with pc = min(p, value).  pc = 4 is Aarseth's formula; for
  *                 p = 8 it uses only a, j, s, c, all direct force-kernel outputs (no 1/h^k noise amplification).
  *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
- *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 4, 16, 64, 128)
+ *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 8, 32, 128)
  */
 int nbody_set_option(nbody_ctx *ctx, const char *key, int64_t value);
 

@@ -429,9 +429,9 @@ template <int ORDER, int DIFF>
 force_fn pick(int jl) {
     switch (jl) {
         case 1: return k_force<ORDER, 1, DIFF>;
-        case 4: return k_force<ORDER, 4, DIFF>;
-        case 16: return k_force<ORDER, 16, DIFF>;
-        case 64: return k_force<ORDER, 64, DIFF>;
+        case 2: return k_force<ORDER, 2, DIFF>;
+        case 8: return k_force<ORDER, 8, DIFF>;
+        case 32: return k_force<ORDER, 32, DIFF>;
         default: return k_force<ORDER, 128, DIFF>;
     }
 }
@@ -452,7 +452,7 @@ size_t smem_for(int order, int diff) {
     return order == 4 ? Geo<4, 1>::SMEM : order == 6 ? Geo<6, 1>::SMEM : Geo<8, 1>::SMEM;
 }
 
-const int kLanes[5] = {1, 4, 16, 64, 128};
+const int kLanes[5] = {1, 2, 8, 32, 128};
 
 }  // namespace
 
@@ -474,11 +474,32 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     // geometry: j-lanes (a CTA owns 2 * 256 / JL i-particles), i-tiles, j-splits
     int jl;
     if (c->force_lanes) jl = c->force_lanes;
-    else jl = n_act > 128 ? 1 : n_act > 32 ? 4 : n_act > 8 ? 16 : n_act > 4 ? 64 : 128;
+    else jl = n_act > 256 ? 1 : n_act > 64 ? 2 : n_act > 16 ? 8 : n_act > 4 ? 32 : 128;
     const int i_per_cta = 2 * (kThreads / jl);
     const int64_t i_tiles = (n_act + i_per_cta - 1) / i_per_cta;
-    const int64_t target = 2 * (int64_t)c->sm_count;  // 2 resident CTAs per SM
-    int64_t S = c->force_split ? c->force_split : (i_tiles >= target ? 1 : (target + i_tiles - 1) / i_tiles);
+    // j-splits: the chip holds `slots` CTAs at once (2 per SM); a launch of i_tiles * S CTAs takes
+    // ceil(i_tiles * S / slots) waves of (n_tiles / S + fixed per-CTA cost) tile-times.  Pick the S that minimises it:
+    // small blocks get S ~ slots / i_tiles (fill the chip), mid-size blocks get a CTA count that is close to a
+    // multiple of `slots` (no half-empty last wave), big blocks (>= 8 waves) run unsplit.
+    const int64_t slots = 2 * (int64_t)c->sm_count;
+    int64_t S = 1;
+    if (c->force_split) {
+        S = c->force_split;
+    } else if (i_tiles < 8 * slots) {
+        const double fixed = 3.0;  // prologue + epilogue + reduce, in tile-times
+        double best = 1e300, cost1 = 0.0;
+        const int64_t s_max = n_tiles < 4 * slots ? n_tiles : 4 * slots;
+        for (int64_t s = 1; s <= s_max; ++s) {
+            const int64_t waves = (i_tiles * s + slots - 1) / slots;
+            const double cost = (double)waves * ((double)((n_tiles + s - 1) / s) + fixed);
+            if (s == 1) cost1 = cost;
+            if (cost < best * (1.0 - 1e-9)) {
+                best = cost;
+                S = s;
+            }
+        }
+        if (best > 0.97 * cost1) S = 1;  // a split costs S x NC x n_act doubles of scratch: only for a real gain
+    }
     if (S > n_tiles) S = n_tiles;
     if (S > 65535) S = 65535;
     if (S < 1) S = 1;
