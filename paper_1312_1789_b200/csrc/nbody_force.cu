@@ -25,6 +25,9 @@
 #ifndef NB_UNROLL
 #define NB_UNROLL 4
 #endif
+#ifndef NB_MINB
+#define NB_MINB 2  // resident CTAs per SM the register budget is sized for
+#endif
 
 namespace nbody {
 namespace {
@@ -272,7 +275,7 @@ __device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const 
 }
 
 template <int ORDER, int JL, int DIFF>
-__global__ void __launch_bounds__(kThreads, 2) k_force(const ForceArgs A) {
+__global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) {
     typedef Geo<ORDER, DIFF> G;
     constexpr int NQ = G::NQ, NC = G::NC, STAGES = G::STAGES;
     constexpr int IT = kThreads / JL;    // threads per j-lane; the CTA owns 2 IT i-particles

@@ -115,7 +115,7 @@ def integrate(args):
     order = args.order or c["order"]
     n, eps2 = c["n"], c["eps2"]
     g = Integrator(c["m"], c["x"], c["v"], order, eps2, eta=args.eta, dt_min=2.0**-args.dt_min_log2,
-                   dt_max=2.0**-4)
+                   dt_max=2.0**-args.dt_max_log2)
     t0 = time.perf_counter()
     g.bootstrap()
     torch.cuda.synchronize()
@@ -156,7 +156,7 @@ def integrate(args):
     e1 = g.energy() if bool((g.t == g.t[0]).all()) else float("nan")
     dts = g.dt.cpu().numpy()
     print(json.dumps({"call": "integrate", "config": args.config, "n": n, "order": order, "eta": args.eta,
-                      "dt_criterion_order": g.dt_criterion_order, "t_end": args.t_end, "reached_t_end": done,
+                      "dt_criterion_order": g.dt_criterion_order, "dt_max_log2": -args.dt_max_log2, "t_end": args.t_end, "reached_t_end": done,
                       "time_reached": g.time, "blocks": g.blocks, "pairs": pairs, "wall_s": wall,
                       "bootstrap_s": t_boot, "split_s": {"predict": t_pred, "force": t_force, "correct": t_corr,
                                                          "host_and_selection": wall - t_pred - t_force - t_corr},
@@ -183,6 +183,7 @@ def main(argv=None):
     i.add_argument("--t-end", type=float, default=0.0625)
     i.add_argument("--eta", type=float, default=0.1)
     i.add_argument("--dt-min-log2", type=int, default=30)
+    i.add_argument("--dt-max-log2", type=int, default=4, help="dt_max = 2^-k (must divide t_end)")
     i.add_argument("--max-seconds", type=float, default=1500.0)
     args = ap.parse_args(argv)
     (sweep if args.cmd == "sweep" else integrate)(args)
