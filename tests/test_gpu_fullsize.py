@@ -5,7 +5,7 @@ seeded draw -- where mixed-precision errors are largest).
   config 4: N = 1 048 576, 6th order, ALL active (the bench.py launch: 2048 CTAs, no j-split)
   config 3: N =   262 144, 6th order, N_act sweep 4^0 .. 4^9 (every lane variant and j-split at full N)
   config 2: N =    65 536, 4th order, N_act = 1, 16, 256, 4096, 65 536
-  config 5: N = 2 097 152, 8th order, ALL active
+  config 5: N = 2 097 152, 8th order, ALL active, and N_act = 3 .. 1.5 M (j-split partials at the largest N)
 """
 import numpy as np
 import pytest
@@ -58,7 +58,8 @@ def test_all_active_full_size_sampled(config, order, sample):
     ctx.close()
 
 
-@pytest.mark.parametrize("config,order,nacts", [(3, 6, [4**k for k in range(10)]), (2, 4, [1, 16, 256, 4096, 65536])])
+@pytest.mark.parametrize("config,order,nacts", [(3, 6, [4**k for k in range(10)]), (2, 4, [1, 16, 256, 4096, 65536]),
+                                                 (5, 8, [3, 1000, 300000, 1500000])])
 def test_nact_sweep_full_size_sampled(config, order, nacts):
     import torch
     c, n, ctx, O, (xp, vp, ap, jp) = _setup(config, order)
