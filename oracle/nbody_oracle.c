@@ -280,7 +280,9 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
  * c-7 interpolated a^(K..2K-1)(t1), Delta = a0 - a1 (formulas below).
  *
  * c-8b: `crit_order` pc in {4, 6, 8}, pc < p, evaluates the c-8 criterion of order pc on a^(0..pc-1)(t1)
- * (0 = order p).  Added after the CUDA path showed that with fp32 pair arithmetic (c-12) the interpolated
+ * (0 = order p).  For p = 6, pc = 4 the fourth entry is the mean crackle of the step (s1 - s0)/h instead of the
+ * interpolated a3 (whose force-noise amplification is 60/h^3), so that, like p = 8, pc = 4, only derivatives the force
+ * call computes directly enter the step decision.  Added after the CUDA path showed that with fp32 pair arithmetic (c-12) the interpolated
  * a^(K..2K-1) of p >= 6 are rounding-noise dominated at small h and the order-p criterion collapses dt.
  *
  * State arrays (in/out, [n][3] unless noted): t[n], dt[n], x, v, D[k] = a^(k)
@@ -303,6 +305,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
         const double h = dt[i];
         const double h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h, h6 = h5 * h, h7 = h6 * h;
         double dnew[8][3];
+        double cbar[3] = {0.0, 0.0, 0.0}; /* c-8b, p = 6: mean crackle over the step, (s1 - s0)/h */
         for (int c = 0; c < 3; ++c) {
             const int64_t q = 3 * i + c, qa = 3 * ia + c;
             const double x0 = x[q], v0 = v[q];
@@ -333,6 +336,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                 const double A5 = (-60.0 * ((((12.0 * dl + (6.0 * h) * j0) + (6.0 * h) * j1) + h2 * s0) - h2 * s1)) / h5;
                 dnew[0][c] = a1; dnew[1][c] = j1; dnew[2][c] = s1;
                 dnew[3][c] = A3; dnew[4][c] = A4; dnew[5][c] = A5;
+                cbar[c] = (s1 - s0) / h;
             } else {
                 const double s0 = D[2][q], s1 = snap[qa];
                 const double c0 = D[3][q], c1 = crackle[qa];
@@ -354,6 +358,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
         }
         const double *dp[8];
         for (int k = 0; k < p; ++k) dp[k] = dnew[k];
+        if (p == 6 && pc == 4) dp[3] = cbar; /* only directly computed derivatives enter the criterion */
         const double dt_new = oracle_new_dt(pc, dp, t_now, h, eta, dt_min, dt_max);
         for (int k = 0; k < p; ++k)
             for (int c = 0; c < 3; ++c) D[k][3 * i + c] = dnew[k][c];

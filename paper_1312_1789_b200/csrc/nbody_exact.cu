@@ -213,6 +213,7 @@ __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
     const double h = A.dt[i];
     const double h2 = M_(h, h), h3 = M_(h2, h), h4 = M_(h3, h), h5 = M_(h4, h), h6 = M_(h5, h), h7 = M_(h6, h);
     double dn[8][3];
+    double cbar[3] = {0.0, 0.0, 0.0};  // R8b, p = 6: mean crackle over the step, (s1 - s0) / h
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const long long q = 3 * i + c, qa = 3 * ia + c;
@@ -238,6 +239,7 @@ __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
             const double A4 = Q_(M_(-12.0, S_(P_(P_(P_(M_(30.0, dl), M_(M_(14.0, h), j0)), M_(M_(16.0, h), j1)), M_(M_(2.0, h2), s0)), M_(M_(3.0, h2), s1))), h4);
             const double A5 = Q_(M_(-60.0, S_(P_(P_(P_(M_(12.0, dl), M_(M_(6.0, h), j0)), M_(M_(6.0, h), j1)), M_(h2, s0)), M_(h2, s1))), h5);
             dn[0][c] = a1; dn[1][c] = j1; dn[2][c] = s1; dn[3][c] = A3; dn[4][c] = A4; dn[5][c] = A5;
+            cbar[c] = Q_(S_(s1, s0), h);
         } else {
             const double s0 = A.D[2][q], s1 = A.snap[qa];
             const double c0 = A.D[3][q], c1 = A.crk[qa];
@@ -260,7 +262,14 @@ __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
         A.v[q] = v1;
     }
     double dt_new;
-    if (ORDER >= 6 && A.crit_order == 4)
+    if (ORDER == 6 && A.crit_order == 4) {  // only directly computed derivatives enter the step decision
+        double d4[4][3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            d4[0][c] = dn[0][c]; d4[1][c] = dn[1][c]; d4[2][c] = dn[2][c]; d4[3][c] = cbar[c];
+        }
+        dt_new = new_dt<4>(d4, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+    } else if (ORDER >= 8 && A.crit_order == 4)
         dt_new = new_dt<4>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
     else if (ORDER >= 8 && A.crit_order == 6)
         dt_new = new_dt<6>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);

@@ -346,7 +346,8 @@ def test_block_timestep_energy_conservation_plummer(order):
 def test_dt_criterion_order_option(order, pc):
     """crit_order pc < p: the corrector's new step equals the order-pc criterion evaluated on the lowest pc
     derivatives at t1 (which the corrector stores, so they can be read back), everything else is untouched;
-    it still reproduces eta/lambda on an exponential, and it differs from the order-p criterion in general."""
+    it still reproduces eta/lambda on an exponential, and it differs from the order-p criterion in general.  For
+    p = 6, pc = 4 the fourth entry is the mean crackle (s1 - s0)/h: only directly computed derivatives decide."""
     rng = np.random.default_rng(8)
     n = 64
     idx = np.arange(n, dtype=np.int32)
@@ -366,7 +367,10 @@ def test_dt_criterion_order_option(order, pc):
     for k in range(order):
         assert np.array_equal(a["D"][k], b["D"][k])
     want_p = np.array([O.new_dt(order, [a["D"][k][i] for k in range(order)], h, h, 0.1, 2.0**-30, 2.0**-2) for i in range(n)])
-    want_pc = np.array([O.new_dt(pc, [a["D"][k][i] for k in range(pc)], h, h, 0.1, 2.0**-30, 2.0**-2) for i in range(n)])
+    low = [a["D"][k] for k in range(pc)]
+    if order == 6 and pc == 4:  # mean crackle of the step from the two directly computed snaps
+        low[3] = (f[2] - base["D"][2]) / h
+    want_pc = np.array([O.new_dt(pc, [low[k][i] for k in range(pc)], h, h, 0.1, 2.0**-30, 2.0**-2) for i in range(n)])
     assert np.array_equal(a["dt"], want_p)
     assert np.array_equal(b["dt"], want_pc)
     assert np.any(want_p != want_pc)
