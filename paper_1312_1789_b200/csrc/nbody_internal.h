@@ -16,8 +16,14 @@ namespace nbody {
 // order 4 reads Q0..Q2, order 6 and 8 read Q0..Q3; diff_mode 1 reads Q4, Q5 instead of Q0, Q1.  The force kernel
 // feeds a j-value to both lanes of a packed f32x2 instruction as a broadcast 32-bit register operand.  Entries [n, n_pad) are zero-mass pads parked far away.
 constexpr int kPlanes = 6;
-constexpr int kTileJ = 128;    // j-particles per TMA stage (and the padding granule of the j-store)
-constexpr int kThreads = 256;  // threads per force CTA
+#ifndef NB_TILEJ
+#define NB_TILEJ 256
+#endif
+constexpr int kTileJ = NB_TILEJ;  // j-particles per TMA stage (and the padding granule of the j-store)
+#ifndef NB_THREADS
+#define NB_THREADS 512
+#endif
+constexpr int kThreads = NB_THREADS;  // threads per force CTA
 constexpr double kPadPos = 1.0e6;
 
 struct Ctx {

@@ -2,7 +2,7 @@
 oracle computes one by one (forced members: every BH, innermost / outermost particles, nearest to each BH, plus a
 seeded draw -- where mixed-precision errors are largest).
 
-  config 4: N = 1 048 576, 6th order, ALL active (the bench.py launch: 2048 CTAs, no j-split)
+  config 4: N = 1 048 576, 6th order, ALL active (the bench.py launch: 1024 CTAs of 512 threads, no j-split)
   config 3: N =   262 144, 6th order, N_act sweep 4^0 .. 4^9 (every lane variant and j-split at full N)
   config 2: N =    65 536, 4th order, N_act = 1, 16, 256, 4096, 65 536
   config 5: N = 2 097 152, 8th order, ALL active, and N_act = 3 .. 1.5 M (j-split partials at the largest N)
@@ -48,7 +48,7 @@ def test_all_active_full_size_sampled(config, order, sample):
     idx_all = torch.arange(n, dtype=torch.int32, device="cuda")
     out = _force(ctx, idx_all, n, order, c["eps2"])
     g = ctx.last_force_geometry()
-    assert g["j_lanes"] == 1 and g["j_splits"] == 1 and g["ctas"] == (n + 511) // 512  # the configuration bench.py times
+    assert g["j_lanes"] == 1 and g["j_splits"] == 1 and g["ctas"] == (n + 1023) // 1024  # the configuration bench.py times
     s = W.oracle_sample(c, size=sample)
     ref = O.force(c["m"], xp, vp, ap, jp, s, order, c["eps2"])
     ii = torch.from_numpy(s.astype(np.int64)).cuda()
