@@ -44,7 +44,8 @@ int nbody_abi_version(void);
 const char *nbody_strerror(int code);
 
 /* Create a context for up to n_capacity particles on CUDA device `device`.  Allocates the packed j-store
- * (4 planes x 16 B x n_capacity rounded up to the j-tile), the split-partial scratch and small control
+ * (6 planes x 16 B x n_capacity rounded up to the 256-particle j-tile; 4 of them in use unless diff_mode is 1), the
+ * selection scratch and small control
  * blocks with cudaMalloc.  *out is set only on success.  Synchronises the device. */
 int nbody_create(nbody_ctx **out, int64_t n_capacity, int device);
 

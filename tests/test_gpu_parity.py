@@ -168,3 +168,33 @@ def test_force_double_single_mode(nb, O):
     got = U.gpu_force(ctx, n, order, c["eps2"], 0.0, t, c["m"], c["x"], c["v"], D, idx)
     U.check_force(got, ref, order, "double-single")
     ctx.close()
+
+
+def test_force_degenerate_inputs(nb, O):
+    """Empty inputs are no-ops; a DIFFERENT particle at the identical position is included (R2): with eps2 > 0 it
+    adds exactly 0 to acc/jerk/snap and -m/eps to pot; zero-mass particles contribute exactly nothing."""
+    import torch
+    ctx = nb.Context(64)
+    z3, z1 = U.zeros(8, 3), U.zeros(8)
+    ctx.predict(0, 0.0, 4, None, None, None, None, [None, None])  # n == 0
+    ctx.force(None, 0, 4, 1e-4, None, None, None, None, None)     # n_act == 0
+    eps2 = 1e-4
+    m = np.array([0.3, 0.2, 0.0, 0.5])
+    x = np.array([[0.1, 0.2, 0.3], [0.1, 0.2, 0.3], [0.4, -0.1, 0.0], [-1.0, 0.5, 0.25]])  # 0 and 1 coincide
+    v = np.array([[0.0, 0.1, 0.0], [0.0, 0.1, 0.0], [3.0, 2.0, 1.0], [0.2, 0.0, -0.1]])
+    D = [np.zeros((4, 3)) for _ in range(6)]
+    t = np.zeros(4)
+    idx = np.arange(4, dtype=np.int32)
+    got = U.gpu_force(ctx, 4, 6, eps2, 0.0, t, m, x, v, D, idx)
+    ref = O.force(m, x, v, D[0], D[1], idx, 6, eps2)
+    U.check_force(got, ref, 6, "coincident pair")
+    # particle 0 sees particle 1 only through the potential: acc equals the pull of particle 3 alone
+    only3 = O.force(m[[0, 3]], x[[0, 3]], v[[0, 3]], D[0][[0, 3]], D[1][[0, 3]], np.array([0], dtype=np.int32), 6, eps2)
+    assert np.allclose(got[0][0], only3[0][0], rtol=1e-6)
+    assert np.isclose(got[4][0], only3[4][0] - m[1] / np.sqrt(eps2), rtol=1e-6)
+    # the zero-mass particle 2 changes nobody's result
+    wo = U.gpu_force(ctx, 3, 6, eps2, 0.0, t[:3], m[[0, 1, 3]], x[[0, 1, 3]], v[[0, 1, 3]], [d[:3] for d in D], idx[:3])
+    for a, b in zip(got, wo):
+        if a is not None:
+            assert np.array_equal(a[[0, 1, 3]], b)
+    ctx.close()
