@@ -58,10 +58,11 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
 /* Tuning / evidence knobs (host-side integers; unknown key -> NBODY_EINVAL).
  *   "diff_mode"   0 = literal: d = fl32(x_j - x_i), subtraction in fp64 (DADD + F2F)          [default]
  *                 1 = double-single: x = hi + lo (two fp32), d = (hi_j - hi_i) + (lo_j - lo_i)  (R10 note)
- *   "dt_criterion_order" 0 = criterion of the scheme's own order p (R8)                        [default]
- *                 4 | 6 = R8b: evaluate the same criterion family on the lowest 4 (6) derivatives only, i.e.
- *                 dt = eta (A^(1)/A^(pc-2))^(1/(pc-3)) with pc = min(p, value).  pc = 4 is Aarseth's formula; for
- *                 p = 8 it uses only a, j, s, c, all direct force-kernel outputs (no 1/h^k noise amplification).
+ *   "dt_criterion_order" pc: dt = eta (A^(1)/A^(pc-2))^(1/(pc-3)) evaluated on the lowest pc derivatives at t_now.
+ *                 0 = automatic [default]: pc = p for order 4, pc = 4 (Aarseth's formula) for orders 6 and 8 (R8b:
+ *                 only derivatives the force call computes directly decide the step; for p = 6 the fourth entry is
+ *                 the mean crackle (s1 - s0)/h).  4 | 6 | 8 = pc = min(p, value); value = p is the order-p
+ *                 criterion of R8, which fp32 force noise collapses for p >= 6 (R8b): fp64 forces only.
  *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
  *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 8, 32, 128)
  */

@@ -619,7 +619,8 @@ int nbody_correct(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int or
     CorrArgs A;
     A.idx = active_idx; A.n_act = n_act; A.t_now = t_now; A.eta = eta; A.dt_min = dt_min; A.dt_max = dt_max;
     A.k_min = kmin; A.k_max = kmax;
-    A.crit_order = (c->crit_order && c->crit_order < order) ? c->crit_order : order;
+    // 0 = automatic: R8b (pc = 4) for p >= 6, where the order-p criterion collapses under fp32 force noise
+    A.crit_order = c->crit_order ? (c->crit_order < order ? c->crit_order : order) : (order >= 6 ? 4 : order);
     A.t = t; A.dt = dt; A.x = x; A.v = v; A.pot_state = pot_state;
     for (int k = 0; k < 8; ++k) A.D[k] = k < order ? a_derivs[k] : nullptr;
     A.acc = acc; A.jerk = jerk; A.snap = snap; A.crk = crackle; A.pot = pot;

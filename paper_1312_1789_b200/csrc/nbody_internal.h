@@ -53,7 +53,7 @@ struct Ctx {
     int diff_mode = 0;
     int force_split = 0;
     int force_lanes = 0;
-    int crit_order = 0;  // 0 = the scheme's own order (R8); 4 or 6 = R8b
+    int crit_order = 0;  // 0 = automatic (4 for p >= 6, else p); 4 | 6 | 8 = criterion order min(p, value) (R8 / R8b)
     // bookkeeping
     int last_cuda_error = 0;
     int64_t launches = 0;

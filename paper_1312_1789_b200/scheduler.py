@@ -12,9 +12,9 @@ from . import nbody
 class Integrator:
     def __init__(self, m, x, v, order, eps2, eta=0.1, eta_s=0.01, dt_min=2.0**-30, dt_max=2.0**-4, device=0,
                  ctx=None, dt_criterion_order=None):
-        """dt_criterion_order: None = 4 for order >= 6 (R8b: with fp32 pair arithmetic the order-p
-        criterion of R8 is driven by rounding noise in the interpolated derivatives and collapses the steps; Aarseth's
-        four-derivative formula is stable), 0 = the order-p criterion of R8, else 4 | 6."""
+        """dt_criterion_order: None / 0 = the library's automatic choice (pc = 4 for order >= 6, R8b: with
+        fp32 pair arithmetic the order-p criterion of R8 is driven by rounding noise in the interpolated derivatives
+        and collapses the steps); 4 | 6 | 8 = criterion order min(order, value) (value = order: R8)."""
         assert order in (4, 6, 8)
         self.order, self.eps2, self.eta, self.eta_s = order, float(eps2), float(eta), float(eta_s)
         self.dt_min, self.dt_max = float(dt_min), float(dt_max)
@@ -22,10 +22,8 @@ class Integrator:
         n = int(np.asarray(m).shape[0])
         self.n = n
         self.ctx = ctx if ctx is not None else nbody.Context(n, device)
-        if dt_criterion_order is None:
-            dt_criterion_order = 4 if order >= 6 else 0
-        self.dt_criterion_order = int(dt_criterion_order)
-        self.ctx.set_option("dt_criterion_order", self.dt_criterion_order)
+        self.ctx.set_option("dt_criterion_order", int(dt_criterion_order or 0))
+        self.dt_criterion_order = int(dt_criterion_order) if dt_criterion_order else (4 if order >= 6 else order)
         up = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.dev)
         self.m, self.x, self.v = up(m), up(x), up(v)
         z = lambda *s: torch.zeros(*s, dtype=torch.float64, device=self.dev)

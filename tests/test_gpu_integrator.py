@@ -54,7 +54,7 @@ def test_correct_bit_exact(nb, O, order, crit):
         gD = [U.dev(d) for d in D]
         gpot = U.zeros(n)
         ctx = nb.Context(n)
-        ctx.set_option("dt_criterion_order", crit)
+        ctx.set_option("dt_criterion_order", crit if crit else order)  # 0 would mean "automatic" (R8b for p >= 6)
         ctx.correct(U.dev(idx), idx.shape[0], order, t_now, eta, 2.0**-30, 2.0**-4, gt, gdt, gx, gv, gD, gpot,
                     U.dev(acc), U.dev(jerk), None if snap is None else U.dev(snap),
                     None if crk is None else U.dev(crk), U.dev(pot))
