@@ -64,7 +64,7 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 the mean crackle (s1 - s0)/h).  4 | 6 | 8 = pc = min(p, value); value = p is the order-p
  *                 criterion of R8, which fp32 force noise collapses for p >= 6 (R8b): fp64 forces only.
  *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
- *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 8, 32, 128)
+ *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 4, 8, 32, 128)
  */
 int nbody_set_option(nbody_ctx *ctx, const char *key, int64_t value);
 

@@ -453,6 +453,7 @@ force_fn pick(int jl) {
     switch (jl) {
         case 1: return k_force<ORDER, 1, DIFF>;
         case 2: return k_force<ORDER, 2, DIFF>;
+        case 4: return k_force<ORDER, 4, DIFF>;
         case 8: return k_force<ORDER, 8, DIFF>;
         case 32: return k_force<ORDER, 32, DIFF>;
         default: return k_force<ORDER, 128, DIFF>;
@@ -475,7 +476,8 @@ size_t smem_for(int order, int diff) {
     return order == 4 ? Geo<4, 1>::SMEM : order == 6 ? Geo<6, 1>::SMEM : Geo<8, 1>::SMEM;
 }
 
-const int kLanes[5] = {1, 2, 8, 32, 128};
+constexpr int kNumLanes = 6;
+const int kLanes[kNumLanes] = {1, 2, 4, 8, 32, 128};
 
 }  // namespace
 
@@ -483,7 +485,7 @@ int force_static_init(Ctx *c) {
     const int orders[3] = {4, 6, 8};
     for (int diff = 0; diff < 2; ++diff)
         for (int o = 0; o < 3; ++o)
-            for (int j = 0; j < 5; ++j)
+            for (int j = 0; j < kNumLanes; ++j)
                 NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, kLanes[j]),
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                 (int)smem_for(orders[o], diff)));
@@ -499,7 +501,7 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     if (c->force_lanes) jl = c->force_lanes;
     else {  // the most j-lanes whose CTA still holds all active particles (2 * kThreads / JL i-slots)
         jl = 1;
-        for (int k = 4; k >= 1; --k)
+        for (int k = kNumLanes - 1; k >= 1; --k)
             if ((int64_t)2 * kThreads / kLanes[k] >= n_act) { jl = kLanes[k]; break; }
     }
     const int i_per_cta = 2 * (kThreads / jl);
