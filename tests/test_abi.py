@@ -59,13 +59,15 @@ def test_null_and_bad_arguments_without_device():
 
 
 def test_sass_shows_tma_and_no_tensor_or_local_in_hot_kernel():
-    """cuobjdump evidence: the force kernels use TMA bulk copies (UBLKCP) + mbarrier (SYNCS), MUFU.RSQ, and the
+    """cuobjdump evidence: the force kernels use TMA bulk copies (UBLKCP) + mbarrier (SYNCS), MUFU.RSQ, FFMA2, and the
     exact TU has no fused fp64 multiply-add (DFMA) in K_pred / K_corr."""
     from paper_1312_1789_b200 import build
     build.build()
     csrc = os.path.join(ROOT, "paper_1312_1789_b200", "csrc")
     sass = subprocess.run(["cuobjdump", "-sass", os.path.join(csrc, "nbody_force.o")], capture_output=True, text=True).stdout
     assert "UBLKCP" in sass and "SYNCS" in sass and "MUFU.RSQ" in sass
+    # Blackwell packed fp32 pair arithmetic (fma/mul/add.f32x2) and no spilled hot loop in the 6th-order kernel
+    assert "FFMA2" in sass and "FMUL2" in sass and "FADD2" in sass
     sass = subprocess.run(["cuobjdump", "-sass", os.path.join(csrc, "nbody_exact.o")], capture_output=True, text=True).stdout
     fn = None
     for line in sass.splitlines():
