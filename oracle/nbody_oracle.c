@@ -23,8 +23,10 @@
  * mpmath brute force on N <= 8, circular two-body closed form, Sum m a = 0 ...
  * Sum m c = 0, Plummer W -> -1/2, polynomial exactness of predictor /
  * corrector / interpolated derivatives, exponential dt pin eta/lambda,
- * quantisation properties, convergence slopes 4/6/8 (table B2), Kepler closure,
- * energy conservation.  Parity unpinned: nothing.
+ * quantisation against exact rational arithmetic (ties and one-ulp near-ties
+ * included), the c-8b mean-crackle criterion against its closed form for
+ * a(t) = a0 e^(lambda t) (50-digit mpmath), convergence slopes 4/6/8 (table B2),
+ * Kepler closure, energy conservation.  Parity unpinned: nothing.
  */
 #include <math.h>
 #include <stddef.h>
@@ -279,8 +281,10 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
  *        x1 = x0 + h/2 (v0+v1) + 3h^2/28 (a0-a1) + h^3/84 (j0+j1) + h^4/1680 (s0-s1)
  * c-7 interpolated a^(K..2K-1)(t1), Delta = a0 - a1 (formulas below).
  *
- * c-8b: `crit_order` pc in {4, 6, 8}, pc < p, evaluates the c-8 criterion of order pc on a^(0..pc-1)(t1)
- * (0 = order p).  For p = 6, pc = 4 the fourth entry is the mean crackle of the step (s1 - s0)/h instead of the
+ * c-8b: `crit_order` selects the criterion order pc.  0 = automatic, the same meaning as the CUDA library's
+ * "dt_criterion_order" option value 0 (include/nbody.h): pc = p for p = 4, pc = 4 for p >= 6.  4 | 6 | 8 = pc =
+ * min(p, value), so value = p is the order-p criterion of c-8.  The order-pc criterion is evaluated on
+ * a^(0..pc-1)(t1).  For p = 6, pc = 4 the fourth entry is the mean crackle of the step (s1 - s0)/h instead of the
  * interpolated a3 (whose force-noise amplification is 60/h^3), so that, like p = 8, pc = 4, only derivatives the force
  * call computes directly enter the step decision.  Added after the CUDA path showed that with fp32 pair arithmetic (c-12) the interpolated
  * a^(K..2K-1) of p >= 6 are rounding-noise dominated at small h and the order-p criterion collapses dt.
@@ -296,9 +300,12 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                     const double *crackle, const double *pot, int variant, int crit_order)
 {
     const int p = order;
-    /* c-8b (R8b): the criterion may be evaluated on the lowest pc <= p derivatives only
-     * (crit_order 0 = p, the c-8 reading).  pc = 4 is Aarseth's formula on a, j, a2, a3. */
-    const int pc = (crit_order == 4 || crit_order == 6 || crit_order == 8) && crit_order < p ? crit_order : p;
+    /* c-8b (R8b): the criterion may be evaluated on the lowest pc <= p derivatives only.
+     * crit_order 0 = automatic (pc = 4 for p >= 6, else p); 4 | 6 | 8 = min(p, value); value = p is c-8.
+     * pc = 4 is Aarseth's formula on a, j, a2, a3. */
+    const int pc = (crit_order == 4 || crit_order == 6 || crit_order == 8)
+                       ? (crit_order < p ? crit_order : p)
+                       : (p >= 6 ? 4 : p);
 #pragma omp parallel for schedule(static)
     for (int64_t ia = 0; ia < n_act; ++ia) {
         const int64_t i = active_idx[ia];

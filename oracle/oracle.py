@@ -112,7 +112,9 @@ def initial_dt(acc, jerk, eta_s, dt_min, dt_max):
 
 def correct(active_idx, order, t_now, eta, dt_min, dt_max, t, dt, x, v, D, pot_state, acc, jerk, snap, crackle, pot,
             variant=0, crit_order=0):
-    """c-6..c-9 (+ c-8b crit_order), IN PLACE on t, dt, x, v, D[0..order-1], pot_state (all must be C-contiguous float64 arrays)."""
+    """c-6..c-9 (+ c-8b crit_order), IN PLACE on t, dt, x, v, D[0..order-1], pot_state (all must be C-contiguous float64
+    arrays).  crit_order: 0 = automatic (criterion order 4 for order >= 6, else the order), the same meaning as the
+    library's "dt_criterion_order" 0; 4 | 6 | 8 = min(order, value) (value = order: the order-p criterion of c-8)."""
     idx = np.ascontiguousarray(active_idx, dtype=np.int32)
     for a in (t, dt, x, v, pot_state, *D[:order]):
         assert a.dtype == np.float64 and a.flags.c_contiguous

@@ -30,7 +30,7 @@ def _state(config, n, order, seed_stream=11):
     return c, D, t, dt
 
 
-@pytest.mark.parametrize("order,crit", [(4, 0), (6, 0), (8, 0), (6, 4), (8, 4), (8, 6)])
+@pytest.mark.parametrize("order,crit", [(4, 0), (6, 0), (8, 0), (4, 4), (6, 6), (8, 8), (6, 4), (8, 4), (8, 6)])
 def test_correct_bit_exact(nb, O, order, crit):
     import torch
     n = 3001
@@ -54,7 +54,7 @@ def test_correct_bit_exact(nb, O, order, crit):
         gD = [U.dev(d) for d in D]
         gpot = U.zeros(n)
         ctx = nb.Context(n)
-        ctx.set_option("dt_criterion_order", crit if crit else order)  # 0 would mean "automatic" (R8b for p >= 6)
+        ctx.set_option("dt_criterion_order", crit)  # same value, same meaning on both sides (0 = automatic, R8b)
         ctx.correct(U.dev(idx), idx.shape[0], order, t_now, eta, 2.0**-30, 2.0**-4, gt, gdt, gx, gv, gD, gpot,
                     U.dev(acc), U.dev(jerk), None if snap is None else U.dev(snap),
                     None if crk is None else U.dev(crk), U.dev(pot))

@@ -205,13 +205,161 @@ def test_dt_quantisation_properties():
             assert math.fmod(t1, got) == 0.0
             if got > dt_min:
                 assert got <= crit * (1 + 1e-12)
-            want = 2.0 ** math.floor(math.log2(crit))
-            want = min(want, 2 * dt_old)
-            if want == 2 * dt_old and math.fmod(t1, want) != 0.0:
-                want = dt_old
-            want = max(min(want, dt_max), dt_min)
-            if abs(math.log2(crit) - round(math.log2(crit))) > 1e-9:
-                assert got == want
+            # the quantised value itself is pinned without any skipped case in test_dt_quantisation_exact_rational
+
+
+
+def _norm3(d):
+    """|d| in fp64 in the order c-8 states ((x^2 + y^2) + z^2, IEEE sqrt): python floats are IEEE fp64."""
+    return math.sqrt((float(d[0]) * float(d[0]) + float(d[1]) * float(d[1])) + float(d[2]) * float(d[2]))
+
+
+def _exact_k(order, derivs, eta):
+    """c-9 step 1 with exact rational arithmetic: the largest integer k with Ap 2^(k q) <= fl(A1 E), where A1, Ap,
+    E are the fp64 numbers c-8/c-9 define (norms, sqrt, E = eta^q by repeated fp64 products) and everything from
+    there on is exact (fractions.Fraction: no log, no pow, no ldexp search, no rounding).  None if Ap == 0."""
+    q = order - 3
+    n = [_norm3(d) for d in derivs]
+    A1 = math.sqrt(n[0] * n[2] + n[1] * n[1])
+    Ap = math.sqrt(n[order - 3] * n[order - 1] + n[order - 2] * n[order - 2])
+    E = 1.0
+    for _ in range(q):
+        E = E * eta
+    rhs = A1 * E
+    if Ap == 0.0:
+        return None
+    ratio = Fraction(rhs) / Fraction(Ap)  # exact
+    if ratio <= 0:
+        return -10**9
+    # largest k with 2^(k q) <= ratio
+    k = (ratio.numerator.bit_length() - ratio.denominator.bit_length()) // q + 2
+    while Fraction(2) ** (k * q) > ratio:
+        k -= 1
+    return k
+
+
+def _quantise(k, t1, dt_old, dt_min, dt_max):
+    """c-9 steps 2-4 on exact dyadic numbers."""
+    kmin, kmax = int(round(math.log2(dt_min))), int(round(math.log2(dt_max)))
+    want = Fraction(2) ** max(min(k, kmax + 1), kmin - 1) if k is not None else Fraction(2) ** (kmax + 1)
+    two_old = 2 * Fraction(dt_old)
+    want = min(want, two_old)
+    if want == two_old and (Fraction(t1) / want).denominator != 1:
+        want = Fraction(dt_old)
+    want = min(want, Fraction(dt_max))
+    want = max(want, Fraction(dt_min))
+    return float(want)
+
+
+def test_dt_quantisation_exact_rational():
+    """c-9 against exact rational arithmetic (no tolerance, no skipped case): 2400 random derivative sets for
+    p = 4, 6, 8, plus constructed ties and one-ulp near-ties where a log2-based floor would go wrong."""
+    rng = np.random.default_rng(11)
+    dt_min, dt_max = 2.0**-24, 2.0**-2
+    for order in (4, 6, 8):
+        for _ in range(800):
+            derivs = [rng.normal(0, 1, 3) * 10.0 ** rng.uniform(-2, 2) * 25.0**k for k in range(order)]
+            kold = int(rng.integers(-20, -3))
+            dt_old = 2.0**kold
+            t1 = dt_old * int(rng.integers(1, 1000))
+            eta = float(rng.choice([0.1, 0.02, 0.3, 2.0**-3]))
+            got = O.new_dt(order, derivs, t1, dt_old, eta, dt_min, dt_max)
+            want = _quantise(_exact_k(order, derivs, eta), t1, dt_old, dt_min, dt_max)
+            assert got == want, (order, eta, derivs)
+    # constructed ties and near-ties: derivatives along x with |a^(k)| = lambda^k => A1/Ap = lambda^-(q) * (exact
+    # powers of two), dt_crit = eta / lambda; eta one ulp either side of a power of two flips the floor
+    ex = np.array([1.0, 0.0, 0.0])
+    for order in (4, 6, 8):
+        for lam_log2 in (0, 1, 3):
+            lam = 2.0**lam_log2
+            derivs = [ex * lam**k for k in range(order)]
+            for k_eta in (-3, -5):
+                e0 = 2.0**k_eta
+                for eta, kk in ((e0, k_eta - lam_log2), (np.nextafter(e0, 0.0), k_eta - lam_log2 - 1),
+                                (np.nextafter(e0, 1.0), k_eta - lam_log2)):
+                    assert _exact_k(order, derivs, float(eta)) == kk
+                    got = O.new_dt(order, derivs, 0.0, 2.0**kk, float(eta), 2.0**-40, 1.0)
+                    assert got == 2.0**kk, (order, lam, eta)
+
+
+def test_dt_mean_crackle_closed_form_pin():
+    """c-8b, p = 6 with the 4-derivative criterion (the library default, R8b): for a(t) = a0 e^(lambda t)
+    the mean crackle of the step is cbar = (s1 - s0)/h = lambda^2 a1 (1 - e^(-lambda h))/h = lambda^2 a1 g, so
+    A^(1) = sqrt(2) lambda |a1|, A^(2) = lambda^(3/2) |a1| sqrt(g + lambda) and
+        dt_crit = eta sqrt(2 / (lambda (g + lambda)))        (-> eta/lambda as h -> 0),
+    evaluated here with 50-digit mpmath and quantised by hand; the oracle never sees this formula.  The cases
+    include ones where the true crackle (dt_crit = eta/lambda) and the interpolated a3 of c-7 would land on a
+    different power of two, so a corrector that fed either of those to the criterion fails."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    u = np.array([0.6, -0.48, 0.64])  # unit vector
+    discriminates_true, discriminates_interp, sens_half, sens_double = 0, 0, 0, 0
+    cases = [(52.0, 0.1, -6), (40.0, 0.1, -6), (90.0, 0.1, -7), (11.0, 0.05, -5), (300.0, 0.2, -8), (23.0, 0.1, -5),
+             (6.5, 0.1, -3), (52.78, 0.1, -8), (26.4, 0.05, -7), (105.5, 0.2, -9), (13.2, 0.1, -6), (3.3, 0.1, -4)]
+    for lam, eta, hlog in cases:
+        h = 2.0**hlog
+        a0n = 0.37
+        L, H = mp.mpf(lam), mp.mpf(h)
+        g = (1 - mp.e ** (-L * H)) / H
+        crit = mp.mpf(eta) * mp.sqrt(2 / (L * (g + L)))
+        lg = mp.log(crit, 2)
+        assert abs(lg - mp.nint(lg)) > mp.mpf("1e-6")  # the case does not sit on a power-of-two boundary
+        k = int(mp.floor(lg))
+        assert 2.0**k < 2 * h  # no doubling limit in play
+        # state at t0 and "force" at t1 = h: exact exponential derivatives
+        e1 = math.exp(lam * h)
+        D = [np.ascontiguousarray((a0n * lam**kk) * u[None, :]) for kk in range(6)] + [np.zeros((1, 3)), np.zeros((1, 3))]
+        f = [np.ascontiguousarray((a0n * lam**kk * e1) * u[None, :]) for kk in range(3)]
+        t, dt = np.zeros(1), np.full(1, h)
+        x, v, ps = np.zeros((1, 3)), np.zeros((1, 3)), np.zeros(1)
+        for crit_order in (4, 0):  # explicit and automatic mean the same thing for p = 6
+            tt, dd = t.copy(), dt.copy()
+            DD = [d.copy() for d in D]
+            O.correct(np.array([0], dtype=np.int32), 6, h, eta, 2.0**-40, 1.0, tt, dd, x.copy(), v.copy(), DD, ps.copy(),
+                      f[0], f[1], f[2], None, np.zeros(1), crit_order=crit_order)
+            assert dd[0] == 2.0**k, (lam, eta, h, dd[0], 2.0**k)
+        # what the other two candidate fourth entries would have produced (mpmath, c-7's a3 formula)
+        k_true = int(mp.floor(mp.log(mp.mpf(eta) / L, 2)))
+        a1 = mp.mpf(a0n) * mp.e ** (L * H)
+        a0m, j0, s0 = mp.mpf(a0n), mp.mpf(a0n) * L, mp.mpf(a0n) * L**2
+        j1, s1 = a1 * L, a1 * L**2
+        a3 = -3 * (20 * (a0m - a1) + 8 * H * j0 + 12 * H * j1 + H**2 * s0 - 3 * H**2 * s1) / H**3
+        crit_i = mp.mpf(eta) * mp.sqrt((a1 * s1 + j1**2) / (j1 * abs(a3) + s1**2))
+        k_int = int(mp.floor(mp.log(crit_i, 2)))
+        discriminates_true += k_true != k
+        discriminates_interp += k_int != k
+        # a factor-2 slip in cbar (e.g. dividing by 2h, or h/2) must change the result in several cases
+        for scale, which in ((mp.mpf("0.5"), "half"), (mp.mpf(2), "double")):
+            km = int(mp.floor(mp.log(mp.mpf(eta) * mp.sqrt(2 / (L * (scale * g + L))), 2)))
+            if which == "half":
+                sens_half += km != k
+            else:
+                sens_double += km != k
+    assert discriminates_true >= 2 and discriminates_interp >= 1, (discriminates_true, discriminates_interp)
+    assert sens_half >= 3 and sens_double >= 1, (sens_half, sens_double)
+
+
+def test_dt_criterion_automatic_option_value():
+    """crit_order 0 = automatic = the library's "dt_criterion_order" 0 (include/nbody.h): order p for p = 4, the
+    4-derivative criterion for p = 6, 8.  Checked by equality with the explicit values on random inputs."""
+    rng = np.random.default_rng(21)
+    n = 32
+    idx = np.arange(n, dtype=np.int32)
+    h = 2.0**-6
+    mk = lambda: np.ascontiguousarray(rng.normal(0, 1, (n, 3)))
+    for order, same_as, differs_from in ((4, 4, None), (6, 4, 6), (8, 4, 8)):
+        base = dict(x=mk(), v=mk(), D=[mk() * 3.0**k for k in range(8)])
+        f = [mk() * 3.0**k for k in range(4)]
+        res = {}
+        for co in {0, same_as, differs_from or same_as}:
+            t, dt = np.zeros(n), np.full(n, h)
+            x, v, D = base["x"].copy(), base["v"].copy(), [d.copy() for d in base["D"]]
+            O.correct(idx, order, h, 0.1, 2.0**-30, 2.0**-2, t, dt, x, v, D, np.zeros(n), f[0], f[1],
+                      f[2] if order >= 6 else None, f[3] if order >= 8 else None, np.zeros(n), crit_order=co)
+            res[co] = dt
+        assert np.array_equal(res[0], res[same_as])
+        if differs_from:
+            assert np.any(res[0] != res[differs_from])
 
 
 def test_dt_degenerate_cases():
@@ -333,7 +481,7 @@ def test_block_timestep_energy_conservation_plummer(order):
     dt_min, dt_max = 2.0**-24, 2.0**-5
     s = OI.bootstrap(c["m"], c["x"], c["v"], order, eps2, dt_min=dt_min, dt_max=dt_max)
     e0 = OI.total_energy(s, eps2)
-    nb, pairs = OI.integrate(s, 0.125, eps2, 0.1, dt_min, dt_max)
+    nb, pairs = OI.integrate(s, 0.125, eps2, 0.1, dt_min, dt_max, crit_order=order)  # c-8, order-p criterion
     assert np.all(s.t == 0.125)
     assert nb > 4
     assert np.all(np.fmod(s.t, s.dt) == 0.0)
@@ -356,13 +504,13 @@ def test_dt_criterion_order_option(order, pc):
     base = dict(t=np.zeros(n), dt=np.full(n, h), x=mk(), v=mk(), D=[mk() * 3.0**k for k in range(8)], pot=np.zeros(n))
     f = [mk() * 3.0**k for k in range(4)]
     out = {}
-    for co in (0, pc):
+    for co in (order, pc):  # value = order: the order-p criterion of c-8 (0 would mean "automatic", R8b)
         s = dict(t=base["t"].copy(), dt=base["dt"].copy(), x=base["x"].copy(), v=base["v"].copy(),
                  D=[d.copy() for d in base["D"]], pot=base["pot"].copy())
         O.correct(idx, order, h, 0.1, 2.0**-30, 2.0**-2, s["t"], s["dt"], s["x"], s["v"], s["D"], s["pot"],
                   f[0], f[1], f[2], f[3], np.zeros(n), crit_order=co)
         out[co] = s
-    a, b = out[0], out[pc]
+    a, b = out[order], out[pc]
     assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["v"], b["v"])
     for k in range(order):
         assert np.array_equal(a["D"][k], b["D"][k])
