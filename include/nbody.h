@@ -12,10 +12,15 @@
  *   - G = 1, potential negative, one Plummer softening eps2 for all pairs (R3, R11).
  *   - `order` p is 4, 6 or 8; K = p/2 force derivatives (acc, jerk | +snap | +crackle).
  *   - Unless a parameter is marked HOST, every array pointer is a DEVICE pointer into caller-owned memory,
- *     fp64, contiguous; 3-vectors are row-major [n][3].  `stream` is a cudaStream_t passed as void* (NULL =
- *     the legacy default stream).  Device-pointer calls only enqueue work and return; they never synchronise.
- *   - The ctx owns scratch only (packed j-store, split partials, staging for the *_host calls).  It never frees
- *     or keeps caller memory.  A ctx is bound to the device given at creation and is not thread-safe.
+ *     fp64, contiguous, 8-byte aligned (int32 arrays 4-byte aligned; anything else is NBODY_EINVAL); 3-vectors are
+ *     row-major [n][3].  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     nbody_predict / nbody_force / nbody_correct / nbody_initial_dt / nbody_get_predicted / nbody_pack_rows /
+ *     nbody_unpack_rows only enqueue work and return: they never synchronise and never allocate (all scratch is sized
+ *     in nbody_create).  Calls that return a value to the host say so (nbody_next_block, nbody_run_blocks, *_host);
+ *     with the "validate" option on, nbody_force and nbody_correct also synchronise (debug mode).
+ *   - The ctx owns scratch only (packed j-store, split partials, control block, staging for the *_host calls).  It
+ *     never frees or keeps caller memory.  A ctx is bound to the device given at creation: every call switches to that
+ *     device and restores the caller's current device on return.  A ctx is not thread-safe.
  *   - Every call returns an int status: NBODY_OK (0) or a negative NBODY_E* code; nothing aborts, throws or
  *     prints.  nbody_strerror() maps a code to a static string.
  *   - There is no CPU fallback anywhere: without a CUDA device nbody_create() returns NBODY_ECUDA.
@@ -30,7 +35,8 @@ extern "C" {
 #endif
 
 #define NBODY_OK       0
-#define NBODY_EINVAL  (-1) /* bad argument: order, sizes, NULL where required, eps2 < 0, misalignment          */
+#define NBODY_EINVAL  (-1) /* bad argument: order, sizes, NULL where required, eps2 < 0, misaligned pointer,
+                              dt range, a failed "validate" check                                              */
 #define NBODY_ESTATE  (-2) /* call order: force before predict, force order > order of the last predict       */
 #define NBODY_ECUDA   (-3) /* a CUDA runtime call or launch failed; see nbody_last_cuda_error()               */
 #define NBODY_ENOMEM  (-4) /* device or host allocation failed                                                */
@@ -43,11 +49,16 @@ int nbody_abi_version(void);
 /* Static description of `code`; never NULL. */
 const char *nbody_strerror(int code);
 
-/* Create a context for up to n_capacity particles on CUDA device `device`.  Allocates the packed j-store
- * (6 planes x 16 B x n_capacity rounded up to the 256-particle j-tile; 4 of them in use unless diff_mode is 1), the
- * selection scratch and small control
- * blocks with cudaMalloc.  *out is set only on success.  Synchronises the device. */
+/* Create a context for up to n_capacity particles on CUDA device `device`.  Allocates, with cudaMalloc, the packed
+ * j-store (6 planes x 16 B x n_capacity rounded up to the 256-particle j-tile; 4 of them in use unless diff_mode is
+ * 1), the j-split scratch (rows of 13 doubles: max(4 SMs x 1024, 4 n_capacity) rows, at most 512 MB; the split
+ * heuristic never asks for more, so nbody_force never allocates) and small control blocks.  *out is set only on
+ * success.  Synchronises the device; the caller's current device is left unchanged. */
 int nbody_create(nbody_ctx **out, int64_t n_capacity, int device);
+
+/* Device bytes nbody_create(n_capacity) allocates on a 148-SM part (j-store + split scratch + control blocks);
+ * -1 for an invalid capacity.  HOST arithmetic only. */
+int64_t nbody_workspace_bytes(int64_t n_capacity);
 
 /* Free everything the ctx owns (synchronises the device first).  NULL is a no-op. */
 int nbody_destroy(nbody_ctx *ctx);
@@ -63,8 +74,17 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 only derivatives the force call computes directly decide the step; for p = 6 the fourth entry is
  *                 the mean crackle (s1 - s0)/h).  4 | 6 | 8 = pc = min(p, value); value = p is the order-p
  *                 criterion of R8, which fp32 force noise collapses for p >= 6 (R8b): fp64 forces only.
- *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence)
+ *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence); a forced S
+ *                 with S * n_act beyond the split scratch makes nbody_force return NBODY_EINVAL
  *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 4, 8, 32, 128)
+ *   "geometry_n_act" 0 = the call's n_act decides the j-lane variant and the j-split [default]; G > 0 = decide as if the
+ *                 call had G active particles (G >= n_act).  An i-sharded rank passes its slice of the active list and
+ *                 G = the size of the whole block: every particle is then summed in exactly the order of the unsharded
+ *                 call, so the shards reproduce it bit for bit.
+ *   "validate"    0 = off [default]; 1 = debug mode: nbody_force checks on the device that active_idx is strictly
+ *                 ascending (hence unique) and in [0, n), nbody_correct additionally that t[i] + dt[i] == t_now for
+ *                 every active i; a violation returns NBODY_EINVAL before any arithmetic.  Synchronises `stream`.
+ *   "use_graph"   1 = nbody_run_blocks replays its five launches as one CUDA graph [default]; 0 = plain launches
  */
 int nbody_set_option(nbody_ctx *ctx, const char *key, int64_t value);
 
@@ -98,10 +118,17 @@ int nbody_predict(nbody_ctx *ctx, int64_t n, double t_now, int order,
  *   fp32 pair arithmetic (MUFU rsqrt), per-thread fp32 partial sums over <= 64 consecutive j, then fp64.
  *   Outputs are in ACTIVE-LIST order: acc, jerk, snap, crackle [n_act][3], pot [n_act], fully overwritten.
  *   snap may be NULL when order < 6, crackle when order < 8 (they are not written then).
- *   active_idx: device int32 [n_act], each in [0, n), unique (ascending recommended, not required).
- *   Deterministic: the same inputs and options give bit-identical outputs run to run.
- * Errors: EINVAL (order, n_act < 0, n_act > n, eps2 < 0 or NaN, NULL required pointer), ESTATE (no predict yet,
- * or order > the order of the last predict).  n_act == 0 is a successful no-op.
+ *   active_idx: device int32 [n_act], each in [0, n), unique (ascending recommended, not required; checked only
+ *   with the "validate" option, otherwise an out-of-range index reads out of bounds).
+ *   Deterministic: the same inputs and options give bit-identical outputs run to run, and the result for a particle
+ *   depends on (j-lane variant, j-split) only, never on the other members of the active list.
+ *   Coincident particles: a DIFFERENT particle at the same position is included (R2); with eps2 > 0 it adds exactly 0
+ *   to acc/jerk/snap/crackle and -m/eps to pot; with eps2 == 0 the pair term is 0 x inf and the outputs of both
+ *   particles are NaN (undefined by the method; not an error code).  The zero-mass pads that fill the last j-tile are
+ *   excluded by index, so no real particle can collide with them.
+ * Errors: EINVAL (order, n_act < 0, n_act > n, eps2 < 0 or NaN, 0 < eps2 < 1.18e-38 (flushes to 0 in fp32), NULL or
+ * misaligned pointer, validation failure), ESTATE (no predict yet, or order > the order of the last predict).
+ * n_act == 0 is a successful no-op.
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_force(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order, double eps2,
                 double *acc, double *jerk, double *snap, double *crackle, double *pot, void *stream);
@@ -118,8 +145,10 @@ int nbody_force(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int or
  *   fp64, no FMA contraction, IEEE div/sqrt, operation order as DESIGN.md section 3 states: bit-exact vs oracle.
  *   acc .. pot are the force-call outputs in active-list order.  a_derivs is a HOST array of 8 device pointers,
  *   entries 0 .. order-1 required.  dt_min, dt_max must be exact powers of two.
- * Errors: EINVAL (order, n_act < 0, NULL required pointer, eta <= 0, dt_min/dt_max not powers of two or
- * dt_min > dt_max).  n_act == 0 is a successful no-op.
+ * Errors: EINVAL (order, n_act < 0, NULL or misaligned pointer, eta <= 0, dt_min/dt_max not powers of two or
+ * dt_min > dt_max, (max(|log2 dt_min|, |log2 dt_max|) + 1) (pc - 3) > 1022 for the criterion order pc in use (the
+ * exact power-of-two comparison of R9 stays inside the fp64 exponent range), validation failure).
+ * n_act == 0 is a successful no-op.
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_correct(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order,
                   double t_now, double eta, double dt_min, double dt_max,
@@ -131,6 +160,7 @@ int nbody_correct(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int 
 /* ------------------------------------------------------------------------------------------------------------
  * nbody_initial_dt -- start-up step of the bootstrap (R9b = SURVEY c-10): dt_i = 2^floor(log2(eta_s |a|/|j|))
  * clamped to [dt_min, dt_max]; |j| == 0 -> dt_max.  acc, jerk, dt: device [n][3], [n][3], [n].  Bit-exact.
+ * Errors: EINVAL (n < 0, eta_s <= 0, dt_min/dt_max not powers of two, dt_min > dt_max, |log2| > 1021, NULL pointer).
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double *jerk,
                      double eta_s, double dt_min, double dt_max, double *dt, void *stream);
@@ -139,6 +169,7 @@ int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double 
  * nbody_next_block -- a-1, block selection on the device (R9c = SURVEY c-11): t_next = min_i (t[i] + dt[i])
  * (exact for dyadic values); active = { i : t[i] + dt[i] == t_next } ascending.  Writes active_idx (device
  * int32, capacity n) and returns t_next and n_act through HOST pointers; this call synchronises `stream`.
+ * One kernel (a persistent grid with two grid barriers: min | count | ordered write).
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
                      int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);
@@ -175,16 +206,54 @@ int nbody_step_host(nbody_ctx *ctx, int64_t n, int order, double eps2, double et
                     double *t_next_host, int64_t *n_act_host, int64_t *h2d_bytes, int64_t *d2h_bytes);
 
 /* ------------------------------------------------------------------------------------------------------------
- * nbody_probe_peak -- chip micro-probes used for the roofline denominators.  Runs a
- * register-only loop of one instruction class on every SM for about `millis` ms and returns the achieved
- * rate in 1e12 thread-operations per second in tera_ops_host[0] (an FFMA counts as ONE operation) and the SM
- * clock in MHz measured inside that kernel (clock64 / globaltimer) in tera_ops_host[1]; HOST array of 2.
- *   kind 0 = FFMA (fp32), 1 = DADD (fp64 add), 2 = F2F (fp64->fp32->fp64 round trip, 2 ops), 3 = MUFU.RSQ,
- *   4 = the literal difference pattern DADD + F2F + FADD (3 ops), 5 = packed FFMA2 with two fresh 64-bit register
- *   operands, 6 = packed FFMA2 with three fresh operands (one FFMA2 = ONE operation = 4 flops).
- * Synchronises.
+ * nbody_run_blocks -- N2, the device-driven block step ("individual hierarchically block time-steps";
+ * PAPER.md:65 eq. (1): the latency term).  Runs whole block steps a-1 .. a-4 (selection, predict, force, correct)
+ * back to back WITHOUT the host learning n_act: the selection kernel leaves t_next, n_act and the force geometry in a
+ * device control block, the other kernels read them there (persistent grids of fixed size), and the five launches of
+ * one block step are replayed as ONE CUDA graph.  The host looks at the control block only every 4 .. 64 block
+ * steps.  A block is executed iff t_next <= t_end, n_act <= max_n_act and fewer than max_blocks blocks have run; the
+ * first block that is not executed ends the run (the state is then exactly the state before that block).
+ * Results are bit-identical to the same blocks run through nbody_next_block + nbody_predict + nbody_force +
+ * nbody_correct (same kernels, same geometry rule).
+ *   state t, dt, m, x, v, a_derivs[0..order-1], pot_state: as nbody_correct (in/out, device).
+ *   active_idx (int32 [n]), acc, jerk, snap, crackle ([n][3]), pot ([n]): caller-owned device scratch of the step.
+ *   res (HOST): blocks executed, pairs = Sum n_act * n, the block that stopped the run (t_next, n_act_next),
+ *   stop_reason (1 = t_next > t_end, 2 = n_act > max_n_act, 3 = max_blocks reached) and the executed blocks counted
+ *   by floor(log2 n_act).
+ * The run executes on a ctx-owned stream ordered after everything queued on `stream`; `stream` is made to wait for the
+ * run.  Synchronises.  Requires diff_mode 0.
+ * Errors: as nbody_correct / nbody_force, plus EINVAL for max_blocks < 0 or max_n_act < 1; ESTATE for diff_mode 1.
  * ---------------------------------------------------------------------------------------------------------- */
-int nbody_probe_peak(nbody_ctx *ctx, int kind, int millis, double *tera_ops_host);
+typedef struct nbody_run_result {
+    int64_t blocks;
+    int64_t pairs;
+    double  t_next;
+    int64_t n_act_next;
+    int32_t stop_reason;
+    int32_t reserved;
+    int64_t hist_log2[40];
+} nbody_run_result;
+
+int nbody_run_blocks(nbody_ctx *ctx, int64_t n, int order, double eps2, double eta, double dt_min, double dt_max,
+                     double t_end, int64_t max_blocks, int64_t max_n_act,
+                     double *t, double *dt, const double *m, double *x, double *v,
+                     double *const a_derivs[8] /* HOST array of device pointers */, double *pot_state,
+                     int32_t *active_idx, double *acc, double *jerk, double *snap, double *crackle, double *pot,
+                     nbody_run_result *res /* HOST */, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_pack_rows / nbody_unpack_rows -- the exchange record of the i-sharded multi-GPU step (
+ * PAPER.md:43 "Both use MPI", eq. (1) beta-term: one exchange per block).  rec[k] = { t, dt, pot_state,
+ * x[3], v[3], a^(0)[3] .. a^(order-1)[3] } of particle idx[k]: 9 + 3 order doubles per row, device memory.
+ * pack gathers the rows of idx[0..n_rows) into rec; unpack scatters rec back into the state arrays.  One kernel
+ * each; between them sits the caller's all-gather (torch.distributed / NCCL).  Only enqueues.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_pack_rows(nbody_ctx *ctx, const int32_t *idx, int64_t n_rows, int order,
+                    const double *t, const double *dt, const double *pot_state, const double *x, const double *v,
+                    const double *const a_derivs[8] /* HOST array of device pointers */, double *rec, void *stream);
+int nbody_unpack_rows(nbody_ctx *ctx, const int32_t *idx, int64_t n_rows, int order,
+                      double *t, double *dt, double *pot_state, double *x, double *v,
+                      double *const a_derivs[8] /* HOST array of device pointers */, const double *rec, void *stream);
 
 /* Kernel launches issued through this ctx since creation (all kernels of this library). */
 int64_t nbody_launch_count(const nbody_ctx *ctx);

@@ -173,6 +173,67 @@ void oracle_force(int64_t n, const double *m,
     }
 }
 
+/* ------------------------------------------------------------------------ *
+ * c-16  Conditioning of the sums of c-1 (diagnostic for the parity reports, SURVEY.md
+ * 7.2 H5): for each active i the sums over j != i of the Euclidean NORMS of
+ * the pair terms, abs_k[ia] = Sum_j |term^(k)_ij| (k = 0 acc, 1 jerk, 2 snap,
+ * 3 crackle; entries above the order are left untouched), so that
+ * kappa_k = abs_k / |Sum_j term^(k)_ij| >= 1 measures the cancellation in the
+ * sum a mixed-precision evaluation has to survive.  Same pair formulas as
+ * oracle_force (c-1), same exclusion by index.
+ * ------------------------------------------------------------------------ */
+void oracle_force_abs(int64_t n, const double *m,
+                      const double *xp, const double *vp, const double *ap, const double *jp,
+                      const int32_t *active_idx, int64_t n_act, int order, double eps2,
+                      double *abs_acc, double *abs_jerk, double *abs_snap, double *abs_crackle)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t ia = 0; ia < n_act; ++ia) {
+        const int64_t i = active_idx[ia];
+        double sA = 0.0, sJ = 0.0, sS = 0.0, sC = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double r[3], v[3], a[3] = {0, 0, 0}, jj[3] = {0, 0, 0};
+            for (int d = 0; d < 3; ++d) {
+                r[d] = xp[3 * j + d] - xp[3 * i + d];
+                v[d] = vp[3 * j + d] - vp[3 * i + d];
+                if (order >= 6) a[d] = ap[3 * j + d] - ap[3 * i + d];
+                if (order >= 8) jj[d] = jp[3 * j + d] - jp[3 * i + d];
+            }
+            const double s2 = (r[0] * r[0] + r[1] * r[1] + r[2] * r[2]) + eps2;
+            const double rinv = 1.0 / sqrt(s2);
+            const double q = m[j] * rinv * rinv * rinv;
+            const double alpha = (r[0] * v[0] + r[1] * v[1] + r[2] * v[2]) / s2;
+            double Ap[3], Jp[3], Sp[3], Cp[3];
+            for (int d = 0; d < 3; ++d) {
+                Ap[d] = q * r[d];
+                Jp[d] = q * v[d] - 3.0 * alpha * Ap[d];
+            }
+            sA += sqrt((Ap[0] * Ap[0] + Ap[1] * Ap[1]) + Ap[2] * Ap[2]);
+            sJ += sqrt((Jp[0] * Jp[0] + Jp[1] * Jp[1]) + Jp[2] * Jp[2]);
+            if (order >= 6) {
+                const double vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+                const double ra = r[0] * a[0] + r[1] * a[1] + r[2] * a[2];
+                const double beta = (vv + ra) / s2 + alpha * alpha;
+                for (int d = 0; d < 3; ++d) Sp[d] = q * a[d] - 6.0 * alpha * Jp[d] - 3.0 * beta * Ap[d];
+                sS += sqrt((Sp[0] * Sp[0] + Sp[1] * Sp[1]) + Sp[2] * Sp[2]);
+                if (order >= 8) {
+                    const double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
+                    const double rj = r[0] * jj[0] + r[1] * jj[1] + r[2] * jj[2];
+                    const double gamma = (3.0 * va + rj) / s2 + alpha * (3.0 * beta - 4.0 * alpha * alpha);
+                    for (int d = 0; d < 3; ++d)
+                        Cp[d] = q * jj[d] - 9.0 * alpha * Sp[d] - 9.0 * beta * Jp[d] - 3.0 * gamma * Ap[d];
+                    sC += sqrt((Cp[0] * Cp[0] + Cp[1] * Cp[1]) + Cp[2] * Cp[2]);
+                }
+            }
+        }
+        abs_acc[ia] = sA;
+        abs_jerk[ia] = sJ;
+        if (order >= 6 && abs_snap) abs_snap[ia] = sS;
+        if (order >= 8 && abs_crackle) abs_crackle[ia] = sC;
+    }
+}
+
 /* Euclidean norm, fixed order ((x^2 + y^2) + z^2) then IEEE sqrt. */
 static double nrm3(const double *a)
 {

@@ -26,6 +26,9 @@ def lib():
         L.oracle_force.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, _dp, _ip, C.c_int64, C.c_int, C.c_double,
                                    _dp, _dp, _dp, _dp, _dp]
         L.oracle_force.restype = None
+        L.oracle_force_abs.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, _dp, _ip, C.c_int64, C.c_int, C.c_double,
+                                       _dp, _dp, _dp, _dp]
+        L.oracle_force_abs.restype = None
         L.oracle_new_dt.argtypes = [C.c_int, C.POINTER(_dp), C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
         L.oracle_new_dt.restype = C.c_double
         L.oracle_initial_dt.argtypes = [C.c_int64, _dp, _dp, C.c_double, C.c_double, C.c_double, _dp]
@@ -95,6 +98,22 @@ def force(m, xp, vp, ap, jp, active_idx, order, eps2):
     lib().oracle_force(n, _p(m), _p(xp), _p(vp), _p(ap), _p(jp), idx.ctypes.data_as(_ip), na, order, float(eps2),
                        _p(acc), _p(jerk), _p(snap), _p(crk), _p(pot))
     return acc, jerk, snap, crk, pot
+
+
+def force_abs(m, xp, vp, ap, jp, active_idx, order, eps2):
+    """c-16: Sum_j |pair term| per active particle for acc, jerk, snap, crackle (None above the order); divide by the
+    norm of oracle force's sum to get the conditioning number kappa >= 1."""
+    m, xp, vp = _d(m), _d(xp), _d(vp)
+    ap = _d(ap) if ap is not None else None
+    jp = _d(jp) if jp is not None else None
+    idx = np.ascontiguousarray(active_idx, dtype=np.int32)
+    n, na = m.shape[0], idx.shape[0]
+    a, j = np.empty(na), np.empty(na)
+    s = np.empty(na) if order >= 6 else None
+    c = np.empty(na) if order >= 8 else None
+    lib().oracle_force_abs(n, _p(m), _p(xp), _p(vp), _p(ap), _p(jp), idx.ctypes.data_as(_ip), na, order, float(eps2),
+                           _p(a), _p(j), _p(s), _p(c))
+    return a, j, s, c
 
 
 def new_dt(order, derivs, t1, dt_old, eta, dt_min, dt_max):

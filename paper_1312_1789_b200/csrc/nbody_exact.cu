@@ -1,5 +1,6 @@
 // libnbody.so, translation unit 1: context management and the fp64 bit-exact kernels
-//   K_pred (a-2), K_corr (a-4), initial dt, block selection (a-1), j-store export, host-buffer path.
+//   K_pred (a-2), K_corr (a-4), initial dt, block selection (a-1), j-store export, row pack/unpack for the multi-GPU
+//   exchange, argument validation, the device-driven block step (nbody_run_blocks) and the host-buffer path.
 // Compiled with -fmad=false; in addition every fp64 operation whose rounding matters is written with the
 // __d*_rn intrinsics, which are never contracted, so the results equal a plain IEEE evaluation in the
 // stated order (R12).  The formulas restate DESIGN.md section 3 (R5..R9); the paper
@@ -22,7 +23,7 @@ __device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a,
 __device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
 __device__ __forceinline__ double dsqrt(double a) { return __dsqrt_rn(a); }
 
-// exact 2^e for e in the normal range
+// exact 2^e for e in the normal range [-1022, 1023] (the callers validate (|k| + 1) q <= 1022 on the host)
 __device__ __forceinline__ double pow2i(int e) { return __longlong_as_double((long long)(e + 1023) << 52); }
 
 struct PredArgs {
@@ -32,6 +33,7 @@ struct PredArgs {
     double t_now;
     long long n, n_pad;
     int write_ds;
+    const Ctl *ctl;  // device-driven step: t_now = ctl->t_next, no-op when the run has stopped (else NULL)
 };
 
 __device__ __forceinline__ uint4 pack_dd(double a, double b) {
@@ -61,11 +63,16 @@ template <int ORDER>
 __global__ void __launch_bounds__(256) k_predict(PredArgs A) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= A.n_pad) return;
+    double t_now = A.t_now;
+    if (A.ctl) {
+        if (A.ctl->stop) return;
+        t_now = A.ctl->t_next;
+    }
     double xp[3];
     float vp[3], ap[3] = {0.f, 0.f, 0.f}, jp[3] = {0.f, 0.f, 0.f}, m32 = 0.f;
     if (i < A.n) {
         constexpr int ND = ORDER - 2;
-        const double tau = dsub(A.t_now, A.t[i]);
+        const double tau = dsub(t_now, A.t[i]);
         double c[9];
 #pragma unroll
         for (int k = 1; k <= 8; ++k) c[k] = ddiv(tau, (double)k);
@@ -203,12 +210,28 @@ struct CorrArgs {
     int crit_order;  // R8b: criterion evaluated on the lowest crit_order derivatives (<= ORDER)
     double *t, *dt, *x, *v, *D[8], *pot_state;
     const double *acc, *jerk, *snap, *crk, *pot;
+    const Ctl *ctl;  // device-driven step: n_act and t_now from the control block (else NULL)
 };
 
 template <int ORDER>
+__device__ __forceinline__ void correct_one(const CorrArgs &A, long long ia, double t_now);
+
+template <int ORDER>
 __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
-    const long long ia = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (ia >= A.n_act) return;
+    long long n_act = A.n_act;
+    double t_now = A.t_now;
+    if (A.ctl) {
+        if (A.ctl->stop) return;
+        n_act = A.ctl->n_act;
+        t_now = A.ctl->t_next;
+    }
+    for (long long ia = (long long)blockIdx.x * blockDim.x + threadIdx.x; ia < n_act;
+         ia += (long long)gridDim.x * blockDim.x)
+        correct_one<ORDER>(A, ia, t_now);
+}
+
+template <int ORDER>
+__device__ __forceinline__ void correct_one(const CorrArgs &A, const long long ia, const double t_now) {
     const long long i = A.idx[ia];
     const double h = A.dt[i];
     const double h2 = M_(h, h), h3 = M_(h2, h), h4 = M_(h3, h), h5 = M_(h4, h), h6 = M_(h5, h), h7 = M_(h6, h);
@@ -268,19 +291,19 @@ __global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
         for (int c = 0; c < 3; ++c) {
             d4[0][c] = dn[0][c]; d4[1][c] = dn[1][c]; d4[2][c] = dn[2][c]; d4[3][c] = cbar[c];
         }
-        dt_new = new_dt<4>(d4, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+        dt_new = new_dt<4>(d4, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
     } else if (ORDER >= 8 && A.crit_order == 4)
-        dt_new = new_dt<4>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+        dt_new = new_dt<4>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
     else if (ORDER >= 8 && A.crit_order == 6)
-        dt_new = new_dt<6>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+        dt_new = new_dt<6>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
     else
-        dt_new = new_dt<ORDER>(dn, A.t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+        dt_new = new_dt<ORDER>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
 #pragma unroll
     for (int k = 0; k < ORDER; ++k)
 #pragma unroll
         for (int c = 0; c < 3; ++c) A.D[k][3 * i + c] = dn[k][c];
     A.pot_state[i] = A.pot[ia];
-    A.t[i] = A.t_now;
+    A.t[i] = t_now;
     A.dt[i] = dt_new;
 }
 
@@ -302,13 +325,15 @@ __global__ void k_initial_dt(long long n, const double *acc, const double *jerk,
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------
-// Block selection (a-1, R9c): min of t + dt, then order-preserving compaction of the particles due at it.
+// Block selection (a-1, R9c) in ONE kernel: min of t + dt, then order-preserving compaction of the particles due
+// at it.  A persistent grid (<= one CTA per SM, all resident) with two grid barriers: [min] | [count] | [write].
+// The last phase also leaves the block time, the block size, the force geometry (force_geometry(), evaluated by
+// 1024 threads in parallel) and the run bookkeeping in the device control block, so that the rest of the block
+// step can be launched without the host knowing n_act (nbody_run_blocks).
 // ---------------------------------------------------------------------------------------------------------
 namespace {
 
-constexpr int kSelThreads = 256;
-constexpr int kSelPerThread = 8;
-constexpr int kSelBlock = kSelThreads * kSelPerThread;  // particles per selection CTA
+constexpr int kSelThreads = 1024;
 
 // order-preserving map double -> uint64 (total order of finite values)
 __device__ __forceinline__ unsigned long long dkey(double v) {
@@ -320,16 +345,52 @@ __device__ __forceinline__ double dunkey(unsigned long long k) {
     return __longlong_as_double((long long)b);
 }
 
-__global__ void k_sel_init(unsigned long long *min_key, long long *n_act) {
-    *min_key = ~0ull;
-    *n_act = 0;
+__device__ __forceinline__ void grid_barrier(SelBar *bar, unsigned grid) {
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned gen = *(volatile unsigned *)&bar->gen;
+        if (atomicAdd(&bar->count, 1u) == grid - 1) {
+            bar->count = 0;
+            __threadfence();
+            atomicAdd(&bar->gen, 1u);
+        } else {
+            while (*(volatile unsigned *)&bar->gen == gen) {}
+        }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
-__global__ void __launch_bounds__(kSelThreads) k_sel_min(long long n, const double *t, const double *dt,
-                                                         unsigned long long *min_key) {
+struct SelArgs {
+    long long n;
+    const double *t, *dt;
+    Ctl *ctl;
+    SelBar *bar;
+    int *counts;          // [grid]
+    int32_t *active_idx;  // [n]
+    // force geometry inputs (force_geometry)
+    int n_tiles, sm_count, force_lanes, force_split;
+    long long rows_budget;
+    // run control
+    int run_mode;         // 0 = plain selection (never stops); 1 = run: honour t_end / max_blocks / max_n_act
+    long long max_n_act;  // run: a block larger than this stops the run (stop = 2) for the host to handle
+};
+
+__global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
+    __shared__ unsigned long long s_key[kSelThreads / 32];
+    __shared__ int s_warp[kSelThreads / 32];
+    __shared__ long long s_base, s_all;
+    const unsigned grid = gridDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long long chunk = (A.n + grid - 1) / grid;
+    const long long c0 = (long long)blockIdx.x * chunk;
+    const long long c1 = c0 + chunk < A.n ? c0 + chunk : A.n;
+
+    // ---- phase 1: min of t + dt (exact for dyadic values) ----
     unsigned long long k = ~0ull;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long ki = dkey(dadd(t[i], dt[i]));
+    for (long long i = c0 + tid; i < c1; i += kSelThreads) {
+        const unsigned long long ki = dkey(__dadd_rn(A.t[i], A.dt[i]));
         k = ki < k ? ki : k;
     }
 #pragma unroll
@@ -337,99 +398,136 @@ __global__ void __launch_bounds__(kSelThreads) k_sel_min(long long n, const doub
         const unsigned long long other = __shfl_xor_sync(0xffffffffu, k, o);
         k = other < k ? other : k;
     }
-    __shared__ unsigned long long sm[kSelThreads / 32];
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = k;
+    if (lane == 0) s_key[warp] = k;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int w = 1; w < kSelThreads / 32; ++w) k = sm[w] < k ? sm[w] : k;
-        atomicMin(min_key, k);
+    if (tid == 0) {
+        for (int w = 1; w < kSelThreads / 32; ++w) k = s_key[w] < k ? s_key[w] : k;
+        atomicMin(&A.ctl->min_key, k);
     }
-}
+    grid_barrier(A.bar, grid);
+    const unsigned long long key = *(volatile unsigned long long *)&A.ctl->min_key;
 
-// counts[b] = number of due particles in chunk b
-__global__ void __launch_bounds__(kSelThreads) k_sel_count(long long n, const double *t, const double *dt,
-                                                           const unsigned long long *min_key, int *counts) {
-    const unsigned long long key = *min_key;
-    const long long base = (long long)blockIdx.x * kSelBlock + (long long)threadIdx.x * kSelPerThread;
-    int c = 0;
-#pragma unroll
-    for (int u = 0; u < kSelPerThread; ++u) {
-        const long long i = base + u;
-        if (i < n && dkey(dadd(t[i], dt[i])) == key) ++c;
-    }
-    c = __reduce_add_sync(0xffffffffu, c);
-    __shared__ int sm[kSelThreads / 32];
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = c;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int s = 0;
-        for (int w = 0; w < kSelThreads / 32; ++w) s += sm[w];
-        counts[blockIdx.x] = s;
-    }
-}
-
-// exclusive scan of counts[0..nb) in place by one CTA; total -> *n_act, t_next -> ret[0]
-__global__ void __launch_bounds__(1024) k_sel_scan(int nb, int *counts, long long *n_act,
-                                                   const unsigned long long *min_key, double *ret) {
-    __shared__ int sm[1024];
-    __shared__ int carry;
-    if (threadIdx.x == 0) carry = 0;
-    __syncthreads();
-    for (int base = 0; base < nb; base += 1024) {
-        const int i = base + threadIdx.x;
-        const int v = i < nb ? counts[i] : 0;
-        sm[threadIdx.x] = v;
-        __syncthreads();
-        for (int o = 1; o < 1024; o <<= 1) {
-            const int add = threadIdx.x >= o ? sm[threadIdx.x - o] : 0;
-            __syncthreads();
-            sm[threadIdx.x] += add;
-            __syncthreads();
-        }
-        if (i < nb) counts[i] = carry + sm[threadIdx.x] - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry += sm[1023];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) {
-        *n_act = carry;
-        ret[0] = dunkey(*min_key);
-        ret[1] = (double)carry;
-    }
-}
-
-__global__ void __launch_bounds__(kSelThreads) k_sel_write(long long n, const double *t, const double *dt,
-                                                           const unsigned long long *min_key, const int *offsets,
-                                                           int32_t *active_idx) {
-    const unsigned long long key = *min_key;
-    const long long base = (long long)blockIdx.x * kSelBlock + (long long)threadIdx.x * kSelPerThread;
-    unsigned flags = 0;
-    int c = 0;
-#pragma unroll
-    for (int u = 0; u < kSelPerThread; ++u) {
-        const long long i = base + u;
-        if (i < n && dkey(dadd(t[i], dt[i])) == key) {
-            flags |= 1u << u;
-            ++c;
+    // ---- phase 2: count the due particles; thread `tid` owns the contiguous run [e0, e1) of its CTA's chunk ----
+    const long long per = (chunk + kSelThreads - 1) / kSelThreads;
+    const long long e0 = c0 + (long long)tid * per < c1 ? c0 + (long long)tid * per : c1;
+    const long long e1 = e0 + per < c1 ? e0 + per : c1;
+    int cnt = 0;
+    unsigned mask = 0;  // due flags of the first 32 elements of the run (longer runs are re-read in phase 3)
+    for (long long i = e0; i < e1; ++i) {
+        const bool due = dkey(__dadd_rn(A.t[i], A.dt[i])) == key;
+        if (due) {
+            ++cnt;
+            if (i - e0 < 32) mask |= 1u << (int)(i - e0);
         }
     }
-    // exclusive scan of c over the CTA (thread order == index order)
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int incl = c;
+    int incl = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const int up = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += up;
     }
-    __shared__ int wsum[kSelThreads / 32];
-    if (lane == 31) wsum[warp] = incl;
+    if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    int woff = 0;
-    for (int w = 0; w < warp; ++w) woff += wsum[w];
-    int pos = offsets[blockIdx.x] + woff + incl - c;
+    if (tid == 0) {
+        int run = 0;
+        for (int w = 0; w < kSelThreads / 32; ++w) {
+            const int v = s_warp[w];
+            s_warp[w] = run;
+            run += v;
+        }
+        A.counts[blockIdx.x] = run;
+    }
+    __syncthreads();
+    const int off_in_cta = s_warp[warp] + incl - cnt;
+    grid_barrier(A.bar, grid);
+
+    // ---- phase 3: global offsets, ordered write, control block ----
+    if (warp == 0) {
+        long long before = 0, all = 0;
+        for (unsigned b = lane; b < grid; b += 32) {
+            const int v = *(volatile int *)&A.counts[b];
+            all += v;
+            if (b < blockIdx.x) before += v;
+        }
 #pragma unroll
-    for (int u = 0; u < kSelPerThread; ++u)
-        if (flags & (1u << u)) active_idx[pos++] = (int32_t)(base + u);
+        for (int o = 16; o > 0; o >>= 1) {
+            before += __shfl_xor_sync(0xffffffffu, before, o);
+            all += __shfl_xor_sync(0xffffffffu, all, o);
+        }
+        if (lane == 0) {
+            s_base = before;
+            s_all = all;
+        }
+    }
+    __syncthreads();
+    long long pos = s_base + off_in_cta;
+    for (long long i = e0; i < e1; ++i) {
+        const bool due = (i - e0 < 32) ? ((mask >> (int)(i - e0)) & 1u) : (dkey(__dadd_rn(A.t[i], A.dt[i])) == key);
+        if (due) A.active_idx[pos++] = (int32_t)i;
+    }
+    if (blockIdx.x != 0) return;
+
+    // CTA 0: block time, size, run control, force geometry (the parallel form of force_geometry()'s search)
+    const long long n_act = s_all;
+    const double t_next = dunkey(key);
+    Ctl *ctl = A.ctl;
+    int stop = 0;
+    if (A.run_mode) {
+        if (t_next > ctl->t_end) stop = 1;
+        else if (n_act > A.max_n_act) stop = 2;
+        else if ((long long)ctl->blocks >= ctl->max_blocks) stop = 3;
+    }
+    ForceGeo g = force_geometry(n_act, A.n_tiles, A.sm_count, A.force_lanes, /*force_split=*/1, A.rows_budget);
+    const long long slots = A.sm_count;
+    long long S = 1;
+    if (A.force_split) S = A.force_split;
+    else if (g.i_tiles < 8 * slots) {
+        long long s_max = A.n_tiles < 4 * slots ? A.n_tiles : 4 * slots;
+        if (n_act > 0 && s_max > A.rows_budget / n_act) s_max = A.rows_budget / n_act;
+        unsigned long long mine = ~0ull;  // (cost << 20) | s : the minimum is the cheapest s, smallest s on ties
+        for (long long sc = 1 + tid; sc <= s_max; sc += kSelThreads) {
+            const long long waves = (g.i_tiles * sc + slots - 1) / slots;
+            const unsigned long long cost = (unsigned long long)(waves * ((A.n_tiles + sc - 1) / sc + 3));
+            const unsigned long long kk = (cost << 20) | (unsigned long long)sc;
+            mine = kk < mine ? kk : mine;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, mine, o);
+            mine = other < mine ? other : mine;
+        }
+        __syncthreads();
+        if (lane == 0) s_key[warp] = mine;
+        __syncthreads();
+        if (tid == 0) {
+            for (int w = 1; w < kSelThreads / 32; ++w) mine = s_key[w] < mine ? s_key[w] : mine;
+            if (mine != ~0ull) {
+                const long long best = (long long)(mine >> 20);
+                const long long cost1 = ((g.i_tiles + slots - 1) / slots) * ((long long)A.n_tiles + 3);
+                S = (long long)(mine & 0xfffffull);
+                if (100 * best > 97 * cost1) S = 1;
+            }
+        }
+    }
+    if (tid == 0) {
+        if (S > A.n_tiles) S = A.n_tiles;
+        if (S > 65535) S = 65535;
+        if (S < 1) S = 1;
+        ctl->t_next = t_next;
+        ctl->n_act = n_act;
+        ctl->jl = g.jl;
+        ctl->splits = (int)S;
+        ctl->i_tiles = g.i_tiles;
+        ctl->stop = stop;
+        ctl->min_key = ~0ull;  // every CTA has read it (second barrier): ready for the next selection
+        if (A.run_mode && !stop) {
+            ctl->blocks += 1;
+            ctl->pairs += (unsigned long long)n_act * (unsigned long long)A.n;
+            int b = 0;
+            while ((n_act >> (b + 1)) != 0) ++b;
+            ctl->hist[b < 39 ? b : 39] += 1;
+        }
+    }
 }
 
 bool is_pow2(double x, int *e) {
@@ -440,18 +538,151 @@ bool is_pow2(double x, int *e) {
     return f == 0.5;
 }
 
+// ---- argument validation on the device ("validate" option): index range, strict ascent, due times -------------
+__global__ void k_validate(const int32_t *idx, long long n_act, long long n, const double *t, const double *dt,
+                           double t_now, int *flag) {
+    for (long long ia = (long long)blockIdx.x * blockDim.x + threadIdx.x; ia < n_act;
+         ia += (long long)gridDim.x * blockDim.x) {
+        const long long i = idx[ia];
+        int bad = 0;
+        if (i < 0 || i >= n) bad = 1;
+        else if (ia > 0 && idx[ia - 1] >= i) bad = 2;
+        else if (t && __dadd_rn(t[i], dt[i]) != t_now) bad = 3;
+        if (bad) atomicMax(flag, bad);
+    }
+}
+
+// ---- packed particle records for the multi-GPU exchange: rec[k] = { t, dt, pot, x[3], v[3], D_0[3] .. }
+struct RowArgs {
+    const int32_t *idx;
+    long long n_rows;
+    int order;
+    double *t, *dt, *pot, *x, *v, *D[8];
+    double *rec;
+};
+
+template <bool PACK>
+__global__ void __launch_bounds__(256) k_rows(const RowArgs A) {
+    const int ncol = 9 + 3 * A.order;
+    const long long tot = A.n_rows * ncol;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < tot; o += (long long)gridDim.x * blockDim.x) {
+        const long long k = o / ncol;
+        const int c = (int)(o % ncol);
+        const long long i = A.idx[k];
+        double *p;
+        if (c == 0) p = A.t + i;
+        else if (c == 1) p = A.dt + i;
+        else if (c == 2) p = A.pot + i;
+        else if (c < 6) p = A.x + 3 * i + (c - 3);
+        else if (c < 9) p = A.v + 3 * i + (c - 6);
+        else p = A.D[(c - 9) / 3] + 3 * i + (c - 9) % 3;
+        if (PACK) A.rec[o] = *p;
+        else *p = A.rec[o];
+    }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------
 // C ABI
 // ---------------------------------------------------------------------------------------------------------
-struct nbody_ctx {
-    Ctx c;
-};
+namespace {
+
+inline bool misaligned(const void *p, size_t a) { return p && ((uintptr_t)p & (a - 1)) != 0; }
+
+// Every fp64 array must be 8-byte aligned, every int32 array 4-byte aligned.
+#define NB_ALIGN8(...)                                          \
+    do {                                                        \
+        const void *ps__[] = {__VA_ARGS__};                     \
+        for (const void *p__ : ps__)                            \
+            if (misaligned(p__, 8)) return NBODY_EINVAL;        \
+    } while (0)
+
+int select_grid(const Ctx *c, int64_t n) {
+    int64_t g = (n + kSelThreads - 1) / kSelThreads;
+    if (g > c->sm_count) g = c->sm_count;
+    return (int)(g < 1 ? 1 : g);
+}
+
+void fill_select(nbody_ctx *h, SelArgs &A, int64_t n, const double *t, const double *dt, int32_t *active_idx,
+                 int run_mode, int64_t max_n_act) {
+    Ctx *c = &h->c;
+    A.n = n; A.t = t; A.dt = dt; A.ctl = c->d_ctl; A.bar = h->d_bar; A.counts = c->d_counts; A.active_idx = active_idx;
+    A.n_tiles = (int)((n + kTileJ - 1) / kTileJ);
+    A.sm_count = c->sm_count; A.force_lanes = c->force_lanes; A.force_split = c->force_split;
+    A.rows_budget = c->partial_rows;
+    A.run_mode = run_mode; A.max_n_act = max_n_act;
+}
+
+int launch_predict(Ctx *c, int64_t n, double t_now, int order, const double *t, const double *m, const double *x,
+                   const double *v, const double *const a_derivs[6], const Ctl *ctl, cudaStream_t st) {
+    PredArgs A;
+    A.t = t; A.m = m; A.x = x; A.v = v;
+    for (int k = 0; k < 6; ++k) A.D[k] = k <= order - 3 ? a_derivs[k] : nullptr;
+    for (int p = 0; p < kPlanes; ++p) A.q[p] = c->jstore + (size_t)p * c->cap_pad;
+    A.t_now = t_now;
+    A.n = n;
+    A.n_pad = c->n_pad;
+    A.write_ds = c->ds_valid ? 1 : 0;
+    A.ctl = ctl;
+    const unsigned grid = (unsigned)((c->n_pad + 255) / 256);
+    if (order == 4) k_predict<4><<<grid, 256, 0, st>>>(A);
+    else if (order == 6) k_predict<6><<<grid, 256, 0, st>>>(A);
+    else k_predict<8><<<grid, 256, 0, st>>>(A);
+    NB_CUDA(c, cudaGetLastError());
+    return NBODY_OK;
+}
+
+// criterion order in use (R8 / R8b) and the exponent range check of R9 (pow2i is exact for |e| <= 1022)
+int criterion_order(const Ctx *c, int order) {
+    return c->crit_order ? (c->crit_order < order ? c->crit_order : order) : (order >= 6 ? 4 : order);
+}
+bool dt_range_ok(int kmin, int kmax, int q) {
+    const long long a = kmin < 0 ? -(long long)kmin : kmin, b = kmax < 0 ? -(long long)kmax : kmax;
+    return ((a > b ? a : b) + 1) * q <= 1022;
+}
+
+int launch_correct(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, double t_now, double eta,
+                   double dt_min, double dt_max, int kmin, int kmax, double *t, double *dt, double *x, double *v,
+                   double *const a_derivs[8], double *pot_state, const double *acc, const double *jerk,
+                   const double *snap, const double *crackle, const double *pot, const Ctl *ctl, cudaStream_t st) {
+    CorrArgs A;
+    A.idx = active_idx; A.n_act = n_act; A.t_now = t_now; A.eta = eta; A.dt_min = dt_min; A.dt_max = dt_max;
+    A.k_min = kmin; A.k_max = kmax;
+    A.crit_order = criterion_order(c, order);
+    A.t = t; A.dt = dt; A.x = x; A.v = v; A.pot_state = pot_state;
+    for (int k = 0; k < 8; ++k) A.D[k] = k < order ? a_derivs[k] : nullptr;
+    A.acc = acc; A.jerk = jerk; A.snap = snap; A.crk = crackle; A.pot = pot;
+    A.ctl = ctl;
+    long long blocks = ctl ? 2LL * c->sm_count : (n_act + 127) / 128;
+    if (blocks > 16LL * c->sm_count) blocks = 16LL * c->sm_count;
+    if (order == 4) k_correct<4><<<(unsigned)blocks, 128, 0, st>>>(A);
+    else if (order == 6) k_correct<6><<<(unsigned)blocks, 128, 0, st>>>(A);
+    else k_correct<8><<<(unsigned)blocks, 128, 0, st>>>(A);
+    NB_CUDA(c, cudaGetLastError());
+    return NBODY_OK;
+}
+
+// "validate" option: device-side check of an active list (and of the due times when t != NULL); synchronises.
+int validate_active(Ctx *c, const int32_t *idx, int64_t n_act, int64_t n, const double *t, const double *dt,
+                    double t_now, cudaStream_t st) {
+    NB_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), st));
+    long long blocks = (n_act + 255) / 256;
+    if (blocks > 8LL * c->sm_count) blocks = 8LL * c->sm_count;
+    k_validate<<<(unsigned)blocks, 256, 0, st>>>(idx, n_act, n, t, dt, t_now, c->d_flag);
+    c->launches += 1;
+    NB_CUDA(c, cudaGetLastError());
+    int flag = 0;
+    NB_CUDA(c, cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    return flag ? NBODY_EINVAL : NBODY_OK;
+}
+
+}  // namespace
 
 extern "C" {
 
-int nbody_abi_version(void) { return 1; }
+int nbody_abi_version(void) { return 2; }
 
 const char *nbody_strerror(int code) {
     switch (code) {
@@ -462,6 +693,17 @@ const char *nbody_strerror(int code) {
         case NBODY_ENOMEM: return "out of memory";
         default: return "unknown nbody error code";
     }
+}
+
+int64_t nbody_workspace_bytes(int64_t n_capacity) {
+    if (n_capacity < 1 || n_capacity > (int64_t)1 << 30) return -1;
+    const int64_t cap_pad = (n_capacity + kTileJ - 1) / kTileJ * kTileJ;
+    // the split scratch depends on the SM count (known at create); this is the bound for a 148-SM part
+    int64_t rows = 4LL * 148 * 2 * kThreads > 4 * n_capacity ? 4LL * 148 * 2 * kThreads : 4 * n_capacity;
+    if (rows * 13 * 8 > (int64_t)512 << 20) rows = ((int64_t)512 << 20) / (13 * 8);
+    const int64_t n_tiles = cap_pad / kTileJ;
+    if (rows > n_tiles * n_capacity) rows = n_tiles * n_capacity;
+    return (int64_t)sizeof(uint4) * kPlanes * cap_pad + rows * 13 * 8 + 4096;
 }
 
 int nbody_create(nbody_ctx **out, int64_t n_capacity, int device) {
@@ -475,21 +717,36 @@ int nbody_create(nbody_ctx **out, int64_t n_capacity, int device) {
     if (!h) return NBODY_ENOMEM;
     Ctx *c = &h->c;
     c->device = device;
+    DeviceGuard guard(device);
     int rc = NBODY_OK;
     do {
         cudaError_t e;
-        if ((e = cudaSetDevice(device)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         cudaDeviceProp prop;
         if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         c->sm_count = prop.multiProcessorCount;
         c->cap = n_capacity;
         c->cap_pad = (n_capacity + kTileJ - 1) / kTileJ * kTileJ;
         if ((e = cudaMalloc(&c->jstore, sizeof(uint4) * kPlanes * c->cap_pad)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        c->counts_cap = (c->cap + kSelBlock - 1) / kSelBlock + 1;
-        if ((e = cudaMalloc(&c->d_counts, sizeof(int) * c->counts_cap)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        if ((e = cudaMalloc(&c->d_min_key, sizeof(unsigned long long))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        if ((e = cudaMalloc(&c->d_nact, sizeof(long long))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        if ((e = cudaMallocHost(&c->h_pinned, 4 * sizeof(double))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        // split scratch, sized ONCE: rows of 13 doubles, S * n_act <= partial_rows for every geometry force_geometry() picks
+        int64_t rows = 4LL * c->sm_count * 2 * kThreads > 4 * n_capacity ? 4LL * c->sm_count * 2 * kThreads : 4 * n_capacity;
+        if (rows * 13 * 8 > (int64_t)512 << 20) rows = ((int64_t)512 << 20) / (13 * 8);
+        const int64_t n_tiles = c->cap_pad / kTileJ;
+        if (rows > n_tiles * n_capacity) rows = n_tiles * n_capacity;  // S <= n_tiles, n_act <= capacity
+        c->partial_rows = rows;
+        c->partials_bytes = (size_t)rows * 13 * sizeof(double);
+        if ((e = cudaMalloc(&c->partials, c->partials_bytes)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&c->d_counts, sizeof(int) * (c->sm_count + 1))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&c->d_ctl, sizeof(Ctl))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&h->d_bar, sizeof(SelBar))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&c->d_flag, sizeof(int))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMallocHost(&c->h_ctl, sizeof(Ctl))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        memset(c->h_ctl, 0, sizeof(Ctl));
+        c->h_ctl->min_key = ~0ull;
+        if ((e = cudaMemcpy(c->d_ctl, c->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMemset(h->d_bar, 0, sizeof(SelBar))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaStreamCreateWithFlags(&h->run_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         rc = force_static_init(c);
         if (rc != NBODY_OK) break;
         if ((e = cudaDeviceSynchronize()) != cudaSuccess) { rc = cuda_fail(c, e); break; }
@@ -505,15 +762,20 @@ int nbody_create(nbody_ctx **out, int64_t n_capacity, int device) {
 int nbody_destroy(nbody_ctx *h) {
     if (!h) return NBODY_OK;
     Ctx *c = &h->c;
-    cudaSetDevice(c->device);
+    DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (h->ev_in) cudaEventDestroy(h->ev_in);
+    if (h->ev_out) cudaEventDestroy(h->ev_out);
+    if (h->run_stream) cudaStreamDestroy(h->run_stream);
     cudaFree(c->jstore);
     cudaFree(c->partials);
     cudaFree(c->d_counts);
-    cudaFree(c->d_min_key);
-    cudaFree(c->d_nact);
+    cudaFree(c->d_ctl);
+    cudaFree(h->d_bar);
+    cudaFree(c->d_flag);
     cudaFree(c->stage);
-    if (c->h_pinned) cudaFreeHost(c->h_pinned);
+    if (c->h_ctl) cudaFreeHost(c->h_ctl);
     cudaGetLastError();
     delete h;
     return NBODY_OK;
@@ -554,6 +816,21 @@ int nbody_set_option(nbody_ctx *h, const char *key, int64_t value) {
         c->force_lanes = (int)value;
         return NBODY_OK;
     }
+    if (!strcmp(key, "geometry_n_act")) {
+        if (value < 0 || value > c->cap) return NBODY_EINVAL;
+        c->geometry_n_act = value;
+        return NBODY_OK;
+    }
+    if (!strcmp(key, "validate")) {
+        if (value != 0 && value != 1) return NBODY_EINVAL;
+        c->validate = (int)value;
+        return NBODY_OK;
+    }
+    if (!strcmp(key, "use_graph")) {
+        if (value != 0 && value != 1) return NBODY_EINVAL;
+        c->use_graph = (int)value;
+        return NBODY_OK;
+    }
     return NBODY_EINVAL;
 }
 
@@ -563,30 +840,18 @@ int nbody_predict(nbody_ctx *h, int64_t n, double t_now, int order, const double
     Ctx *c = &h->c;
     if (n > 0) {
         if (!t || !m || !x || !v || !a_derivs) return NBODY_EINVAL;
+        NB_ALIGN8(t, m, x, v);
         for (int k = 0; k <= order - 3; ++k)
-            if (!a_derivs[k]) return NBODY_EINVAL;
+            if (!a_derivs[k] || misaligned(a_derivs[k], 8)) return NBODY_EINVAL;
     }
+    DeviceGuard guard(c->device);
     c->n = n;
     c->n_pad = (n + kTileJ - 1) / kTileJ * kTileJ;
     c->pred_order = order;
     c->ds_valid = c->diff_mode == 1;
     if (n == 0) return NBODY_OK;
-    PredArgs A;
-    A.t = t; A.m = m; A.x = x; A.v = v;
-    for (int k = 0; k < 6; ++k) A.D[k] = k <= order - 3 ? a_derivs[k] : nullptr;
-    for (int p = 0; p < kPlanes; ++p) A.q[p] = c->jstore + (size_t)p * c->cap_pad;
-    A.t_now = t_now;
-    A.n = n;
-    A.n_pad = c->n_pad;
-    A.write_ds = c->ds_valid ? 1 : 0;
-    cudaStream_t st = (cudaStream_t)stream;
-    const unsigned grid = (unsigned)((c->n_pad + 255) / 256);
-    if (order == 4) k_predict<4><<<grid, 256, 0, st>>>(A);
-    else if (order == 6) k_predict<6><<<grid, 256, 0, st>>>(A);
-    else k_predict<8><<<grid, 256, 0, st>>>(A);
     c->launches += 1;
-    NB_CUDA(c, cudaGetLastError());
-    return NBODY_OK;
+    return launch_predict(c, n, t_now, order, t, m, x, v, a_derivs, nullptr, (cudaStream_t)stream);
 }
 
 int nbody_force(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int order, double eps2, double *acc,
@@ -594,11 +859,19 @@ int nbody_force(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int orde
     if (!h || (order != 4 && order != 6 && order != 8) || n_act < 0) return NBODY_EINVAL;
     Ctx *c = &h->c;
     if (!(eps2 >= 0.0) || isinf(eps2)) return NBODY_EINVAL;
+    if (eps2 > 0.0 && (float)eps2 < 1.17549435e-38f) return NBODY_EINVAL;  // would flush to 0 in the fp32 pair arithmetic
     if (c->n < 0 || order > c->pred_order) return NBODY_ESTATE;
     if (n_act > c->n) return NBODY_EINVAL;
     if (n_act == 0) return NBODY_OK;
     if (!active_idx || !acc || !jerk || !pot || (order >= 6 && !snap) || (order >= 8 && !crackle)) return NBODY_EINVAL;
+    NB_ALIGN8(acc, jerk, snap, crackle, pot);
+    if (misaligned(active_idx, 4)) return NBODY_EINVAL;
     if (c->diff_mode == 1 && !c->ds_valid) return NBODY_ESTATE;
+    DeviceGuard guard(c->device);
+    if (c->validate) {
+        const int rc = validate_active(c, active_idx, n_act, c->n, nullptr, nullptr, 0.0, (cudaStream_t)stream);
+        if (rc != NBODY_OK) return rc;
+    }
     return launch_force(c, active_idx, n_act, order, (float)eps2, acc, jerk, snap, crackle, pot, (cudaStream_t)stream);
 }
 
@@ -610,28 +883,22 @@ int nbody_correct(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int or
     Ctx *c = &h->c;
     int kmin, kmax;
     if (!(eta > 0.0) || !is_pow2(dt_min, &kmin) || !is_pow2(dt_max, &kmax) || dt_min > dt_max) return NBODY_EINVAL;
-    if (kmin < -900 || kmax > 900) return NBODY_EINVAL;
+    if (!dt_range_ok(kmin, kmax, criterion_order(c, order) - 3)) return NBODY_EINVAL;
     if (n_act == 0) return NBODY_OK;
     if (!active_idx || !t || !dt || !x || !v || !a_derivs || !pot_state || !acc || !jerk || !pot) return NBODY_EINVAL;
     if ((order >= 6 && !snap) || (order >= 8 && !crackle)) return NBODY_EINVAL;
+    NB_ALIGN8(t, dt, x, v, pot_state, acc, jerk, snap, crackle, pot);
+    if (misaligned(active_idx, 4)) return NBODY_EINVAL;
     for (int k = 0; k < order; ++k)
-        if (!a_derivs[k]) return NBODY_EINVAL;
-    CorrArgs A;
-    A.idx = active_idx; A.n_act = n_act; A.t_now = t_now; A.eta = eta; A.dt_min = dt_min; A.dt_max = dt_max;
-    A.k_min = kmin; A.k_max = kmax;
-    // 0 = automatic: R8b (pc = 4) for p >= 6, where the order-p criterion collapses under fp32 force noise
-    A.crit_order = c->crit_order ? (c->crit_order < order ? c->crit_order : order) : (order >= 6 ? 4 : order);
-    A.t = t; A.dt = dt; A.x = x; A.v = v; A.pot_state = pot_state;
-    for (int k = 0; k < 8; ++k) A.D[k] = k < order ? a_derivs[k] : nullptr;
-    A.acc = acc; A.jerk = jerk; A.snap = snap; A.crk = crackle; A.pot = pot;
-    cudaStream_t st = (cudaStream_t)stream;
-    const unsigned grid = (unsigned)((n_act + 127) / 128);
-    if (order == 4) k_correct<4><<<grid, 128, 0, st>>>(A);
-    else if (order == 6) k_correct<6><<<grid, 128, 0, st>>>(A);
-    else k_correct<8><<<grid, 128, 0, st>>>(A);
+        if (!a_derivs[k] || misaligned(a_derivs[k], 8)) return NBODY_EINVAL;
+    DeviceGuard guard(c->device);
+    if (c->validate) {
+        const int rc = validate_active(c, active_idx, n_act, c->cap, t, dt, t_now, (cudaStream_t)stream);
+        if (rc != NBODY_OK) return rc;
+    }
     c->launches += 1;
-    NB_CUDA(c, cudaGetLastError());
-    return NBODY_OK;
+    return launch_correct(c, active_idx, n_act, order, t_now, eta, dt_min, dt_max, kmin, kmax, t, dt, x, v, a_derivs,
+                          pot_state, acc, jerk, snap, crackle, pot, nullptr, (cudaStream_t)stream);
 }
 
 int nbody_initial_dt(nbody_ctx *h, int64_t n, const double *acc, const double *jerk, double eta_s, double dt_min,
@@ -639,9 +906,12 @@ int nbody_initial_dt(nbody_ctx *h, int64_t n, const double *acc, const double *j
     if (!h || n < 0) return NBODY_EINVAL;
     int kmin, kmax;
     if (!(eta_s > 0.0) || !is_pow2(dt_min, &kmin) || !is_pow2(dt_max, &kmax) || dt_min > dt_max) return NBODY_EINVAL;
+    if (!dt_range_ok(kmin, kmax, 1)) return NBODY_EINVAL;
     if (n == 0) return NBODY_OK;
     if (!acc || !jerk || !dt) return NBODY_EINVAL;
+    NB_ALIGN8(acc, jerk, dt);
     Ctx *c = &h->c;
+    DeviceGuard guard(c->device);
     k_initial_dt<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(n, acc, jerk, eta_s, kmin, kmax, dt_min,
                                                                               dt_max, dt);
     c->launches += 1;
@@ -652,20 +922,20 @@ int nbody_initial_dt(nbody_ctx *h, int64_t n, const double *acc, const double *j
 int nbody_next_block(nbody_ctx *h, int64_t n, const double *t, const double *dt, int32_t *active_idx,
                      double *t_next_host, int64_t *n_act_host, void *stream) {
     if (!h || n < 1 || n > h->c.cap || !t || !dt || !active_idx || !t_next_host || !n_act_host) return NBODY_EINVAL;
+    NB_ALIGN8(t, dt);
+    if (misaligned(active_idx, 4)) return NBODY_EINVAL;
     Ctx *c = &h->c;
+    DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
-    const int nb = (int)((n + kSelBlock - 1) / kSelBlock);
-    k_sel_init<<<1, 1, 0, st>>>(c->d_min_key, c->d_nact);
-    const int gmin = nb < 4 * c->sm_count ? nb : 4 * c->sm_count;
-    k_sel_min<<<gmin, kSelThreads, 0, st>>>(n, t, dt, c->d_min_key);
-    k_sel_count<<<nb, kSelThreads, 0, st>>>(n, t, dt, c->d_min_key, c->d_counts);
-    k_sel_scan<<<1, 1024, 0, st>>>(nb, c->d_counts, c->d_nact, c->d_min_key, c->h_pinned);
-    k_sel_write<<<nb, kSelThreads, 0, st>>>(n, t, dt, c->d_min_key, c->d_counts, active_idx);
-    c->launches += 5;
+    SelArgs A;
+    fill_select(h, A, n, t, dt, active_idx, /*run_mode=*/0, n);
+    k_select<<<select_grid(c, n), kSelThreads, 0, st>>>(A);
+    c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
+    NB_CUDA(c, cudaMemcpyAsync(c->h_ctl, c->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
     NB_CUDA(c, cudaStreamSynchronize(st));
-    *t_next_host = c->h_pinned[0];
-    *n_act_host = (int64_t)c->h_pinned[1];
+    *t_next_host = c->h_ctl->t_next;
+    *n_act_host = (int64_t)c->h_ctl->n_act;
     return NBODY_OK;
 }
 
@@ -675,6 +945,7 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
     if (c->n < 0) return NBODY_ESTATE;
     if ((ap && c->pred_order < 6) || (jp && c->pred_order < 8)) return NBODY_EINVAL;
     if (c->n == 0) return NBODY_OK;
+    DeviceGuard guard(c->device);
     const uint4 *q = c->jstore;
     k_unpack<<<(unsigned)((c->n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
         q, q + c->cap_pad, q + 2 * c->cap_pad, q + 3 * c->cap_pad, c->n, c->pred_order, xp, vp, ap, jp, m32);
@@ -683,9 +954,169 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
     return NBODY_OK;
 }
 
-int nbody_probe_peak(nbody_ctx *h, int kind, int millis, double *tera_ops_host) {
-    if (!h || !tera_ops_host || kind < 0 || kind > 6 || millis < 1 || millis > 20000) return NBODY_EINVAL;
-    return probe_peak(&h->c, kind, millis, tera_ops_host);
+// ---- row records for the multi-GPU exchange -----------------------------------------------------------------
+static int rows_call(nbody_ctx *h, bool pack, const int32_t *idx, int64_t n_rows, int order, double *t, double *dt,
+                     double *pot_state, double *x, double *v, double *const a_derivs[8], double *rec, void *stream) {
+    if (!h || (order != 4 && order != 6 && order != 8) || n_rows < 0) return NBODY_EINVAL;
+    if (n_rows == 0) return NBODY_OK;
+    if (!idx || !t || !dt || !pot_state || !x || !v || !a_derivs || !rec) return NBODY_EINVAL;
+    NB_ALIGN8(t, dt, pot_state, x, v, rec);
+    RowArgs A;
+    A.idx = idx; A.n_rows = n_rows; A.order = order; A.t = t; A.dt = dt; A.pot = pot_state; A.x = x; A.v = v; A.rec = rec;
+    for (int k = 0; k < 8; ++k) {
+        A.D[k] = k < order ? a_derivs[k] : nullptr;
+        if (k < order && (!a_derivs[k] || misaligned(a_derivs[k], 8))) return NBODY_EINVAL;
+    }
+    Ctx *c = &h->c;
+    DeviceGuard guard(c->device);
+    long long blocks = (n_rows * (9 + 3 * order) + 255) / 256;
+    if (blocks > 8LL * c->sm_count) blocks = 8LL * c->sm_count;
+    if (pack) k_rows<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(A);
+    else k_rows<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(A);
+    c->launches += 1;
+    NB_CUDA(c, cudaGetLastError());
+    return NBODY_OK;
+}
+
+int nbody_pack_rows(nbody_ctx *h, const int32_t *idx, int64_t n_rows, int order, const double *t, const double *dt,
+                    const double *pot_state, const double *x, const double *v, const double *const a_derivs[8],
+                    double *rec, void *stream) {
+    return rows_call(h, true, idx, n_rows, order, (double *)t, (double *)dt, (double *)pot_state, (double *)x, (double *)v,
+                     (double *const *)a_derivs, rec, stream);
+}
+
+int nbody_unpack_rows(nbody_ctx *h, const int32_t *idx, int64_t n_rows, int order, double *t, double *dt,
+                      double *pot_state, double *x, double *v, double *const a_derivs[8], const double *rec,
+                      void *stream) {
+    return rows_call(h, false, idx, n_rows, order, t, dt, pot_state, x, v, a_derivs, (double *)rec, stream);
+}
+
+// ---- device-driven block steps (a-1 .. a-4 without host round trips) ------------------------------------------
+int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta, double dt_min, double dt_max,
+                     double t_end, int64_t max_blocks, int64_t max_n_act, double *t, double *dt, const double *m,
+                     double *x, double *v, double *const a_derivs[8], double *pot_state, int32_t *active_idx,
+                     double *acc, double *jerk, double *snap, double *crackle, double *pot, nbody_run_result *res,
+                     void *stream) {
+    if (!h || (order != 4 && order != 6 && order != 8) || n < 1 || n > h->c.cap || !res) return NBODY_EINVAL;
+    Ctx *c = &h->c;
+    int kmin, kmax;
+    if (!(eta > 0.0) || !is_pow2(dt_min, &kmin) || !is_pow2(dt_max, &kmax) || dt_min > dt_max) return NBODY_EINVAL;
+    if (!dt_range_ok(kmin, kmax, criterion_order(c, order) - 3)) return NBODY_EINVAL;
+    if (!(eps2 >= 0.0) || isinf(eps2) || (eps2 > 0.0 && (float)eps2 < 1.17549435e-38f)) return NBODY_EINVAL;
+    if (max_blocks < 0 || max_n_act < 1 || !(t_end == t_end)) return NBODY_EINVAL;
+    if (!t || !dt || !m || !x || !v || !a_derivs || !pot_state || !active_idx || !acc || !jerk || !pot) return NBODY_EINVAL;
+    if ((order >= 6 && !snap) || (order >= 8 && !crackle)) return NBODY_EINVAL;
+    NB_ALIGN8(t, dt, m, x, v, pot_state, acc, jerk, snap, crackle, pot);
+    if (misaligned(active_idx, 4)) return NBODY_EINVAL;
+    for (int k = 0; k < order; ++k)
+        if (!a_derivs[k] || misaligned(a_derivs[k], 8)) return NBODY_EINVAL;
+    if (c->diff_mode != 0) return NBODY_ESTATE;  // the device-driven step is built for the literal difference mode
+    DeviceGuard guard(c->device);
+    cudaStream_t user = (cudaStream_t)stream, st = h->run_stream;
+    memset(res, 0, sizeof(*res));
+
+    // the private stream runs after everything the caller has queued on `stream`, and the caller's stream resumes
+    // after the run (the legacy default stream cannot be captured into a graph)
+    NB_CUDA(c, cudaEventRecord(h->ev_in, user));
+    NB_CUDA(c, cudaStreamWaitEvent(st, h->ev_in, 0));
+
+    // j-store bookkeeping of the ctx (what nbody_predict would set)
+    c->n = n;
+    c->n_pad = (n + kTileJ - 1) / kTileJ * kTileJ;
+    c->pred_order = order;
+    c->ds_valid = false;
+
+    // run control
+    Ctl *hc = c->h_ctl;
+    memset(hc, 0, sizeof(Ctl));
+    hc->min_key = ~0ull;
+    hc->t_end = t_end;
+    hc->max_blocks = max_blocks;
+    NB_CUDA(c, cudaMemcpyAsync(c->d_ctl, hc, sizeof(Ctl), cudaMemcpyHostToDevice, st));
+
+    SelArgs SA;
+    fill_select(h, SA, n, t, dt, active_idx, /*run_mode=*/1, max_n_act);
+    const int sgrid = select_grid(c, n);
+    auto enqueue_step = [&](cudaStream_t s) -> int {
+        k_select<<<sgrid, kSelThreads, 0, s>>>(SA);
+        NB_CUDA(c, cudaGetLastError());
+        int rc = launch_predict(c, n, 0.0, order, t, m, x, v, a_derivs, c->d_ctl, s);
+        if (rc != NBODY_OK) return rc;
+        rc = launch_force_dyn(c, active_idx, order, (float)eps2, acc, jerk, snap, crackle, pot, s);
+        if (rc != NBODY_OK) return rc;
+        return launch_correct(c, active_idx, 0, order, 0.0, eta, dt_min, dt_max, kmin, kmax, t, dt, x, v, a_derivs,
+                              pot_state, acc, jerk, snap, crackle, pot, c->d_ctl, s);
+    };
+    constexpr int kStepLaunches = 5;  // k_select, k_predict, k_force_dyn, k_reduce_dyn, k_correct
+
+    // one CUDA graph of the five launches, re-captured when any argument differs from the cached one
+    unsigned long long key[24] = {(unsigned long long)n, (unsigned long long)order, 0, 0, 0, 0,
+                                  (unsigned long long)(uintptr_t)t, (unsigned long long)(uintptr_t)dt,
+                                  (unsigned long long)(uintptr_t)m, (unsigned long long)(uintptr_t)x,
+                                  (unsigned long long)(uintptr_t)v, (unsigned long long)(uintptr_t)pot_state,
+                                  (unsigned long long)(uintptr_t)active_idx, (unsigned long long)(uintptr_t)acc,
+                                  (unsigned long long)(uintptr_t)jerk, (unsigned long long)(uintptr_t)snap,
+                                  (unsigned long long)(uintptr_t)crackle, (unsigned long long)(uintptr_t)pot,
+                                  (unsigned long long)max_n_act,
+                                  (unsigned long long)c->crit_order << 32 | (unsigned long long)c->force_lanes << 16 |
+                                      (unsigned long long)c->force_split,
+                                  0, 0, 0, 0};
+    memcpy(&key[2], &eps2, 8); memcpy(&key[3], &eta, 8); memcpy(&key[4], &dt_min, 8); memcpy(&key[5], &dt_max, 8);
+    for (int k = 0; k < order && k < 4; ++k) key[20 + k] = (unsigned long long)(uintptr_t)a_derivs[k];
+    for (int k = 4; k < order; ++k) key[20 + (k & 3)] ^= (unsigned long long)(uintptr_t)a_derivs[k] * 0x9e3779b97f4a7c15ull;
+    if (c->use_graph && (!c->graph_exec || memcmp(key, c->graph_key, sizeof(key)) != 0)) {
+        if (c->graph_exec) {
+            cudaGraphExecDestroy(c->graph_exec);
+            c->graph_exec = nullptr;
+        }
+        cudaGraph_t graph = nullptr;
+        NB_CUDA(c, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+        const int rc = enqueue_step(st);
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        if (rc != NBODY_OK) {
+            if (graph) cudaGraphDestroy(graph);
+            return rc;
+        }
+        NB_CUDA(c, e);
+        const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        NB_CUDA(c, ei);
+        memcpy(c->graph_key, key, sizeof(key));
+    }
+
+    // batches of block steps between two looks at the control block
+    int batch = 4;
+    int rc = NBODY_OK;
+    for (;;) {
+        for (int b = 0; b < batch && rc == NBODY_OK; ++b) {
+            if (c->use_graph) {
+                const cudaError_t e = cudaGraphLaunch(c->graph_exec, st);
+                if (e != cudaSuccess) rc = cuda_fail(c, e);
+            } else {
+                rc = enqueue_step(st);
+            }
+            c->launches += kStepLaunches;
+        }
+        if (rc != NBODY_OK) break;
+        cudaError_t e = cudaMemcpyAsync(hc, c->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if (hc->stop) break;
+        if (batch < 64) batch *= 2;
+    }
+    if (rc != NBODY_OK) {
+        cudaStreamSynchronize(st);
+        return rc;
+    }
+    res->blocks = (int64_t)hc->blocks;
+    res->pairs = (int64_t)hc->pairs;
+    res->t_next = hc->t_next;
+    res->n_act_next = (int64_t)hc->n_act;
+    res->stop_reason = hc->stop;
+    for (int b = 0; b < 40; ++b) res->hist_log2[b] = (int64_t)hc->hist[b];
+    NB_CUDA(c, cudaEventRecord(h->ev_out, st));
+    NB_CUDA(c, cudaStreamWaitEvent(user, h->ev_out, 0));
+    return NBODY_OK;
 }
 
 }  // extern "C"
@@ -693,6 +1124,31 @@ int nbody_probe_peak(nbody_ctx *h, int kind, int millis, double *tera_ops_host) 
 // ---------------------------------------------------------------------------------------------------------
 // Host-buffer path (end-to-end measurement): H2D of the state, predict, force, D2H of the results.
 // ---------------------------------------------------------------------------------------------------------
+namespace {
+// error exit of the *_host calls: drain the stream first, so that no copy from/to caller-owned host memory is in flight
+inline int host_fail(Ctx *c, cudaStream_t st, int rc) {
+    cudaStreamSynchronize(st);
+    (void)c;
+    return rc;
+}
+#define NB_CUDA_H(ctx, st, expr)                                               \
+    do {                                                                       \
+        cudaError_t e__ = (expr);                                              \
+        if (e__ != cudaSuccess) return host_fail(ctx, st, ::nbody::cuda_fail(ctx, e__)); \
+    } while (0)
+
+int ensure_stage(Ctx *c, size_t need) {
+    if (need <= c->stage_bytes) return NBODY_OK;
+    NB_CUDA(c, cudaDeviceSynchronize());
+    cudaFree(c->stage);
+    c->stage = nullptr;
+    c->stage_bytes = 0;
+    NB_CUDA(c, cudaMalloc(&c->stage, need));
+    c->stage_bytes = need;
+    return NBODY_OK;
+}
+}  // namespace
+
 extern "C" int nbody_force_host(nbody_ctx *h, int64_t n, double t_now, int order, const double *t, const double *m,
                                 const double *x, const double *v, const double *const a_derivs[6],
                                 const int32_t *active_idx, int64_t n_act, double eps2, double *acc, double *jerk,
@@ -701,36 +1157,31 @@ extern "C" int nbody_force_host(nbody_ctx *h, int64_t n, double t_now, int order
         return NBODY_EINVAL;
     if (!t || !m || !x || !v || !a_derivs || (n_act > 0 && (!active_idx || !acc || !jerk || !pot))) return NBODY_EINVAL;
     if (n_act > 0 && ((order >= 6 && !snap) || (order >= 8 && !crackle))) return NBODY_EINVAL;
+    if (!(eps2 >= 0.0) || isinf(eps2) || (eps2 > 0.0 && (float)eps2 < 1.17549435e-38f)) return NBODY_EINVAL;
     const int nd = order - 2, K = order / 2;
     for (int k = 0; k < nd; ++k)
         if (!a_derivs[k]) return NBODY_EINVAL;
     Ctx *c = &h->c;
-    NB_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
     // staging layout (doubles): t[n] m[n] x[3n] v[3n] D[nd][3n] | out: K x [3 n_act] + pot[n_act] | idx int32[n_act]
     const size_t in_d = (size_t)n * (2 + 6 + 3 * (size_t)nd);
     const size_t out_d = (size_t)n_act * (3 * (size_t)K + 1);
     const size_t need = (in_d + out_d) * sizeof(double) + (size_t)n_act * sizeof(int32_t) + 256;
-    if (need > c->stage_bytes) {
-        NB_CUDA(c, cudaDeviceSynchronize());
-        cudaFree(c->stage);
-        c->stage = nullptr;
-        c->stage_bytes = 0;
-        NB_CUDA(c, cudaMalloc(&c->stage, need));
-        c->stage_bytes = need;
-    }
+    int rc = ensure_stage(c, need);
+    if (rc != NBODY_OK) return rc;
     cudaStream_t st = 0;
     double *d = (double *)c->stage;
     double *dt_ = d, *dm = d + n, *dx = d + 2 * n, *dv = d + 5 * n;
     const double *dD[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int64_t up = 0, down = 0;
-    NB_CUDA(c, cudaMemcpyAsync(dt_, t, sizeof(double) * n, cudaMemcpyHostToDevice, st));
-    NB_CUDA(c, cudaMemcpyAsync(dm, m, sizeof(double) * n, cudaMemcpyHostToDevice, st));
-    NB_CUDA(c, cudaMemcpyAsync(dx, x, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
-    NB_CUDA(c, cudaMemcpyAsync(dv, v, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
+    NB_CUDA_H(c, st, cudaMemcpyAsync(dt_, t, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    NB_CUDA_H(c, st, cudaMemcpyAsync(dm, m, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    NB_CUDA_H(c, st, cudaMemcpyAsync(dx, x, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
+    NB_CUDA_H(c, st, cudaMemcpyAsync(dv, v, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
     up += (int64_t)sizeof(double) * 8 * n;
     for (int k = 0; k < nd; ++k) {
         double *p = d + 8 * n + (size_t)k * 3 * n;
-        NB_CUDA(c, cudaMemcpyAsync(p, a_derivs[k], sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
+        NB_CUDA_H(c, st, cudaMemcpyAsync(p, a_derivs[k], sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st));
         dD[k] = p;
         up += (int64_t)sizeof(double) * 3 * n;
     }
@@ -741,18 +1192,18 @@ extern "C" int nbody_force_host(nbody_ctx *h, int64_t n, double t_now, int order
     if (order >= 8) { o_crk = cur; cur += 3 * n_act; }
     double *o_pot = cur;
     int32_t *d_idx = (int32_t *)(o + out_d);
-    int rc = nbody_predict(h, n, t_now, order, dt_, dm, dx, dv, dD, st);
-    if (rc != NBODY_OK) return rc;
+    rc = nbody_predict(h, n, t_now, order, dt_, dm, dx, dv, dD, st);
+    if (rc != NBODY_OK) return host_fail(c, st, rc);
     if (n_act > 0) {
-        NB_CUDA(c, cudaMemcpyAsync(d_idx, active_idx, sizeof(int32_t) * n_act, cudaMemcpyHostToDevice, st));
+        NB_CUDA_H(c, st, cudaMemcpyAsync(d_idx, active_idx, sizeof(int32_t) * n_act, cudaMemcpyHostToDevice, st));
         up += (int64_t)sizeof(int32_t) * n_act;
         rc = nbody_force(h, d_idx, n_act, order, eps2, o_acc, o_jerk, o_snap, o_crk, o_pot, st);
-        if (rc != NBODY_OK) return rc;
-        NB_CUDA(c, cudaMemcpyAsync(acc, o_acc, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(c, cudaMemcpyAsync(jerk, o_jerk, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
-        if (order >= 6) NB_CUDA(c, cudaMemcpyAsync(snap, o_snap, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
-        if (order >= 8) NB_CUDA(c, cudaMemcpyAsync(crackle, o_crk, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(c, cudaMemcpyAsync(pot, o_pot, sizeof(double) * n_act, cudaMemcpyDeviceToHost, st));
+        if (rc != NBODY_OK) return host_fail(c, st, rc);
+        NB_CUDA_H(c, st, cudaMemcpyAsync(acc, o_acc, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
+        NB_CUDA_H(c, st, cudaMemcpyAsync(jerk, o_jerk, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
+        if (order >= 6) NB_CUDA_H(c, st, cudaMemcpyAsync(snap, o_snap, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
+        if (order >= 8) NB_CUDA_H(c, st, cudaMemcpyAsync(crackle, o_crk, sizeof(double) * 3 * n_act, cudaMemcpyDeviceToHost, st));
+        NB_CUDA_H(c, st, cudaMemcpyAsync(pot, o_pot, sizeof(double) * n_act, cudaMemcpyDeviceToHost, st));
         down += (int64_t)sizeof(double) * n_act * (3 * K + 1);
     }
     NB_CUDA(c, cudaStreamSynchronize(st));
@@ -774,19 +1225,19 @@ extern "C" int nbody_step_host(nbody_ctx *h, int64_t n, int order, double eps2, 
     for (int k = 0; k < order; ++k)
         if (!a_derivs[k]) return NBODY_EINVAL;
     Ctx *c = &h->c;
-    NB_CUDA(c, cudaSetDevice(c->device));
+    {  // every argument the inner calls would reject is rejected here, before the first copy is queued
+        int kmin, kmax;
+        if (!(eta > 0.0) || !is_pow2(dt_min, &kmin) || !is_pow2(dt_max, &kmax) || dt_min > dt_max) return NBODY_EINVAL;
+        if (!dt_range_ok(kmin, kmax, criterion_order(c, order) - 3)) return NBODY_EINVAL;
+        if (!(eps2 >= 0.0) || isinf(eps2) || (eps2 > 0.0 && (float)eps2 < 1.17549435e-38f)) return NBODY_EINVAL;
+    }
+    DeviceGuard guard(c->device);
     const int K = order / 2;
     // staging (doubles): t dt m pot [n] | x v [3n] | D[order][3n] | acc jerk snap crk [3n] fpot [n] | idx int32[n]
     const size_t nd = (size_t)n * (4 + 6 + 3 * (size_t)order + 12 + 1);
     const size_t need = nd * sizeof(double) + (size_t)n * sizeof(int32_t) + 256;
-    if (need > c->stage_bytes) {
-        NB_CUDA(c, cudaDeviceSynchronize());
-        cudaFree(c->stage);
-        c->stage = nullptr;
-        c->stage_bytes = 0;
-        NB_CUDA(c, cudaMalloc(&c->stage, need));
-        c->stage_bytes = need;
-    }
+    int rc = ensure_stage(c, need);
+    if (rc != NBODY_OK) return rc;
     cudaStream_t st = 0;
     double *d = (double *)c->stage;
     double *d_t = d, *d_dt = d + n, *d_m = d + 2 * n, *d_pot = d + 3 * n, *d_x = d + 4 * n, *d_v = d + 7 * n;
@@ -804,31 +1255,31 @@ extern "C" int nbody_step_host(nbody_ctx *h, int64_t n, int order, double eps2, 
         down += (int64_t)(cnt * sizeof(double));
         return cudaMemcpyAsync(dst, src, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
     };
-    NB_CUDA(c, h2d(d_t, t, n));
-    NB_CUDA(c, h2d(d_dt, dt, n));
-    NB_CUDA(c, h2d(d_m, m, n));
-    NB_CUDA(c, h2d(d_pot, pot_state, n));
-    NB_CUDA(c, h2d(d_x, x, 3 * n));
-    NB_CUDA(c, h2d(d_v, v, 3 * n));
-    for (int k = 0; k < order; ++k) NB_CUDA(c, h2d(d_D[k], a_derivs[k], 3 * n));
+    NB_CUDA_H(c, st, h2d(d_t, t, n));
+    NB_CUDA_H(c, st, h2d(d_dt, dt, n));
+    NB_CUDA_H(c, st, h2d(d_m, m, n));
+    NB_CUDA_H(c, st, h2d(d_pot, pot_state, n));
+    NB_CUDA_H(c, st, h2d(d_x, x, 3 * n));
+    NB_CUDA_H(c, st, h2d(d_v, v, 3 * n));
+    for (int k = 0; k < order; ++k) NB_CUDA_H(c, st, h2d(d_D[k], a_derivs[k], 3 * n));
     double t_next = 0.0;
     int64_t n_act = 0;
-    int rc = nbody_next_block(h, n, d_t, d_dt, d_idx, &t_next, &n_act, st);
-    if (rc != NBODY_OK) return rc;
+    rc = nbody_next_block(h, n, d_t, d_dt, d_idx, &t_next, &n_act, st);
+    if (rc != NBODY_OK) return host_fail(c, st, rc);
     rc = nbody_predict(h, n, t_next, order, d_t, d_m, d_x, d_v, d_D, st);
-    if (rc != NBODY_OK) return rc;
+    if (rc != NBODY_OK) return host_fail(c, st, rc);
     rc = nbody_force(h, d_idx, n_act, order, eps2, o_acc, o_jerk, K >= 3 ? o_snap : nullptr, K >= 4 ? o_crk : nullptr,
                      o_pot, st);
-    if (rc != NBODY_OK) return rc;
+    if (rc != NBODY_OK) return host_fail(c, st, rc);
     rc = nbody_correct(h, d_idx, n_act, order, t_next, eta, dt_min, dt_max, d_t, d_dt, d_x, d_v, d_D, d_pot, o_acc,
                        o_jerk, K >= 3 ? o_snap : nullptr, K >= 4 ? o_crk : nullptr, o_pot, st);
-    if (rc != NBODY_OK) return rc;
-    NB_CUDA(c, d2h(t, d_t, n));
-    NB_CUDA(c, d2h(dt, d_dt, n));
-    NB_CUDA(c, d2h(pot_state, d_pot, n));
-    NB_CUDA(c, d2h(x, d_x, 3 * n));
-    NB_CUDA(c, d2h(v, d_v, 3 * n));
-    for (int k = 0; k < order; ++k) NB_CUDA(c, d2h(a_derivs[k], d_D[k], 3 * n));
+    if (rc != NBODY_OK) return host_fail(c, st, rc);
+    NB_CUDA_H(c, st, d2h(t, d_t, n));
+    NB_CUDA_H(c, st, d2h(dt, d_dt, n));
+    NB_CUDA_H(c, st, d2h(pot_state, d_pot, n));
+    NB_CUDA_H(c, st, d2h(x, d_x, 3 * n));
+    NB_CUDA_H(c, st, d2h(v, d_v, 3 * n));
+    for (int k = 0; k < order; ++k) NB_CUDA_H(c, st, d2h(a_derivs[k], d_D[k], 3 * n));
     NB_CUDA(c, cudaStreamSynchronize(st));
     *t_next_host = t_next;
     *n_act_host = n_act;

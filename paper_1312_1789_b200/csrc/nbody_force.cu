@@ -9,33 +9,31 @@
 //     instruction count of the fp32 part.  The j operand of a packed instruction is the broadcast pair {v, v},
 //     which ptxas folds into a 32-bit broadcast register operand (SASS `Rn.F32`), so the j-store stays compact;
 //   - j-tiles of kTileJ particles are staged plane by plane into shared memory by 1-D TMA bulk copies
-//     (cp.async.bulk + mbarrier) through a ring; every pair-loop read is an LDS.128 broadcast;
+//     (cp.async.bulk + mbarrier) through a 4-stage ring with per-stage full/empty mbarriers (no __syncthreads in
+//     the loop); every pair-loop read is an LDS.128 broadcast;
 //   - d = fl32(x_j - x_i) with the subtraction in fp64 (DIFF 0: DADD + F2F per lane) or double-single (DIFF 1:
 //     packed fp32 adds of hi and lo parts); MUFU.RSQ per lane; fp32 partial sums over <= 64 consecutive j, then
 //     fp64 accumulators, which live in shared memory (one slot per thread and component) to free registers (R10);
-//   - the self pair is excluded by index (R2), but the compare/select is only executed by warps whose i-indices
-//     fall inside the current j-tile (warp-uniform branch), so the main loop is mask-free;
-//   - a CTA is IT = 256/JL i-lanes x JL j-lanes (2 IT i-particles): JL = 1 for big blocks (every lane reads the
-//     same j: smem broadcast), JL up to 256 for tiny blocks; the j-lanes are reduced through shared memory in
-//     fixed order; gridDim.y = S j-splits; S > 1 writes fp64 partials [S][NC][n_act] that K_reduce sums in order.
+//   - the pair is cut into a head (differences, r^2, rsqrt: the LDS -> DADD -> F2F -> MUFU latency chain) and a
+//     tail (the FFMA2 block); at order 8 the heads of two j are issued before their tails (no register spills);
+//   - the self pair (R2) and the zero-mass pads above n are excluded by index, but the compare/select is only
+//     executed by warps whose i-indices fall inside the current j-tile or whose tile holds pads (warp-uniform
+//     branch), so the main loop is mask-free;
+//   - a work item is (i-tile, j-split): IT = kThreads/JL i-lanes x JL j-lanes (2 IT i-particles): JL = 1 for big
+//     blocks (every lane reads the same j: smem broadcast), JL up to 128 for tiny blocks; the j-lanes are reduced
+//     through shared memory in fixed order; S > 1 j-splits write fp64 partials [S][NC][n_act] that K_reduce sums
+//     in order.  k_force takes the geometry from the host (grid = i-tiles x S); k_force_dyn is the persistent
+//     form of the same work items (grid = SMs) that reads n_act and the geometry from the device control block
+//     (device-driven block step, nbody_run_blocks).
 #include <math.h>
 
 #include "nbody_internal.h"
 
-#ifndef NB_UNROLL
-#define NB_UNROLL 4
-#endif
-#ifndef NB_NOBAR
-#define NB_NOBAR 1  // 1 = no __syncthreads per tile: stages are released through per-stage "empty" mbarriers (+1.5 %)
-#endif
-#ifndef NB_MINB
-#define NB_MINB 1  // resident CTAs per SM the register budget is sized for (1 x 512 threads measured 5 % faster than 2 x 256)
-#endif
 
 namespace nbody {
 namespace {
 
-constexpr int kUnroll = NB_UNROLL;  // j-particles per unrolled group of the pair loop
+constexpr int kUnroll = 4;  // j-particles per unrolled group of the pair loop
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -131,12 +129,14 @@ struct Geo {
 struct ForceArgs {
     const uint4 *q[4];  // planes in use: {Q0,Q1,Q2,Q3} (DIFF 0) or {Q4,Q5,Q2,Q3} (DIFF 1)
     const int32_t *idx;
-    int n_act;
+    int n;              // particles in the j-store; entries [n, n_tiles * kTileJ) are pads, masked by index
+    int n_act;          // host-geometry kernel only (k_force_dyn reads it from ctl)
     int n_tiles;
-    int splits;
+    int splits;         // host-geometry kernel only
     float eps2;
-    double *out[5];    // acc, jerk, snap, crackle, pot (used when splits == 1)
-    double *partials;  // [splits][NC][n_act]           (used when splits > 1)
+    double *out[5];     // acc, jerk, snap, crackle, pot (used when splits == 1)
+    double *partials;   // [splits][NC][n_act]           (used when splits > 1)
+    const Ctl *ctl;     // device control block (k_force_dyn)
 };
 
 template <int ORDER, int DIFF>
@@ -149,48 +149,63 @@ struct IPair {          // the thread's two i-particles
 
 struct Consts {  // loop-invariant packed constants
     f2 eps2, m3, three, m4;
+    int n;  // first pad index
 };
 
-// One j against the thread's two i-particles; accumulates into pa[0 .. 3K] (pot as +m/r, negated at the end).
+// One j against the thread's two i-particles, in two parts.  head: d, r^2, rsqrt (LDS, DADD, F2F, FFMA2 x 3, MUFU: the
+// long-latency chain); tail: everything else, accumulating into pa[0 .. 3K] (pot as +m/r, negated at the end).
 // tq = base of the staged tile (plane p at tq + p * kTileJ), jt = index inside the tile.
-template <int ORDER, int DIFF, bool MASK>
-__device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *tq, int jt, int jglob,
-                                      const Consts &C, f2 *pa) {
+struct Stage {
     f2 d[3];
-    const uint4 qa = tq[jt];           // Q0 = { x, y } (f64)           | Q4 = { xhi, xlo, yhi, ylo }
-    const uint4 qb = tq[kTileJ + jt];  // Q1 = { z (f64), m, vx }       | Q5 = { zhi, zlo, m, vx }
+    f2 rinv;
+    unsigned m, vx;
+};
+
+template <int ORDER, int DIFF, bool MASK>
+__device__ __forceinline__ void head(const IPair<ORDER, DIFF> &I, const uint4 *tq, int jt, int jglob, const Consts &C,
+                                     Stage &S) {
+    const uint4 qa = tq[jt];
+    const uint4 qb = tq[kTileJ + jt];
     if (DIFF == 0) {
         const double xj = u2d(qa.x, qa.y), yj = u2d(qa.z, qa.w), zj = u2d(qb.x, qb.y);
-        d[0] = pk(d2f(xj - I.x[0][0]), d2f(xj - I.x[1][0]));
-        d[1] = pk(d2f(yj - I.x[0][1]), d2f(yj - I.x[1][1]));
-        d[2] = pk(d2f(zj - I.x[0][2]), d2f(zj - I.x[1][2]));
+        S.d[0] = pk(d2f(xj - I.x[0][0]), d2f(xj - I.x[1][0]));
+        S.d[1] = pk(d2f(yj - I.x[0][1]), d2f(yj - I.x[1][1]));
+        S.d[2] = pk(d2f(zj - I.x[0][2]), d2f(zj - I.x[1][2]));
     } else {
-        d[0] = add2(add2(bc(qa.x), I.nxh[0]), add2(bc(qa.y), I.nxl[0]));
-        d[1] = add2(add2(bc(qa.z), I.nxh[1]), add2(bc(qa.w), I.nxl[1]));
-        d[2] = add2(add2(bc(qb.x), I.nxh[2]), add2(bc(qb.y), I.nxl[2]));
+        S.d[0] = add2(add2(bc(qa.x), I.nxh[0]), add2(bc(qa.y), I.nxl[0]));
+        S.d[1] = add2(add2(bc(qa.z), I.nxh[1]), add2(bc(qa.w), I.nxl[1]));
+        S.d[2] = add2(add2(bc(qb.x), I.nxh[2]), add2(bc(qb.y), I.nxl[2]));
     }
-    const f2 mj = bc(qb.z);
-    const uint4 qc = tq[2 * kTileJ + jt];  // Q2 = { vy, vz, ax, ay }
-    f2 dv[3], dj[3];
-    dv[0] = add2(bc(qb.w), I.nv[0]);
-    dv[1] = add2(bc(qc.x), I.nv[1]);
-    dv[2] = add2(bc(qc.y), I.nv[2]);
-    f2 da[3];
-    f2 r2 = fma2(d[0], d[0], C.eps2);
-    r2 = fma2(d[1], d[1], r2);
-    r2 = fma2(d[2], d[2], r2);
-    f2 rv = mul2(d[0], dv[0]);
-    rv = fma2(d[1], dv[1], rv);
-    rv = fma2(d[2], dv[2], rv);
+    S.m = qb.z;
+    S.vx = qb.w;
+    f2 r2 = fma2(S.d[0], S.d[0], C.eps2);
+    r2 = fma2(S.d[1], S.d[1], r2);
+    r2 = fma2(S.d[2], S.d[2], r2);
     float r0, r1;
     upk(r2, r0, r1);
     r0 = frsqrt(r0);
     r1 = frsqrt(r1);
-    if (MASK) {
-        r0 = (jglob == I.idx[0]) ? 0.f : r0;
-        r1 = (jglob == I.idx[1]) ? 0.f : r1;
+    if (MASK) {  // R2: the self pair is excluded by index; so are the pads above n
+        r0 = (jglob == I.idx[0] || jglob >= C.n) ? 0.f : r0;
+        r1 = (jglob == I.idx[1] || jglob >= C.n) ? 0.f : r1;
     }
-    const f2 rinv = pk(r0, r1);
+    S.rinv = pk(r0, r1);
+}
+
+template <int ORDER, int DIFF>
+__device__ __forceinline__ void tail(const IPair<ORDER, DIFF> &I, const uint4 *tq, int jt, const Consts &C,
+                                     const Stage &S, f2 *pa) {
+    const f2 *d = S.d;
+    const f2 mj = bc(S.m);
+    const uint4 qc = tq[2 * kTileJ + jt];  // Q2 = { vy, vz, ax, ay }
+    f2 dv[3], dj[3], da[3];
+    dv[0] = add2(bc(S.vx), I.nv[0]);
+    dv[1] = add2(bc(qc.x), I.nv[1]);
+    dv[2] = add2(bc(qc.y), I.nv[2]);
+    f2 rv = mul2(d[0], dv[0]);
+    rv = fma2(d[1], dv[1], rv);
+    rv = fma2(d[2], dv[2], rv);
+    const f2 rinv = S.rinv;
     const f2 rinv2 = mul2(rinv, rinv);
     const f2 mrinv = mul2(mj, rinv);
     const f2 q = mul2(mrinv, rinv2);
@@ -236,7 +251,6 @@ __device__ __forceinline__ void pair2(const IPair<ORDER, DIFF> &I, const uint4 *
             g = fma2(d[0], dj[0], g);
             g = fma2(d[1], dj[1], g);
             g = fma2(d[2], dj[2], g);
-            // gamma = g / s2 + alpha (3 beta - 4 alpha^2)
             const f2 t = fma2(mul2(C.m4, alpha), alpha, mul2(C.three, beta));
             const f2 gamma = fma2(alpha, t, mul2(g, rinv2));
             const f2 c4 = mul2(C.three, c1);  // -9 alpha
@@ -267,46 +281,52 @@ __device__ __forceinline__ void flush(f2 (&pa)[NC], double *acc_mine) {
 template <int ORDER, int JL, int DIFF, bool MASK>
 __device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const uint4 *tq, int j0, int jl,
                                              const Consts &C, f2 (&pa)[3 * (ORDER / 2) + 1], double *acc_mine) {
-    constexpr int JPT = kTileJ / JL;
-    constexpr int CH = JPT < 64 ? JPT : 64;
+    constexpr int JPT = kTileJ / JL;                 // j-particles per thread and tile
+    constexpr int G0 = ORDER == 8 ? 2 : 1;           // heads issued before their tails
+    constexpr int G = G0 < JPT ? G0 : JPT;
+    constexpr int U = (kUnroll < JPT ? kUnroll : JPT) / G;
 #pragma unroll 1
-    for (int jj0 = 0; jj0 < JPT; jj0 += CH) {
-#pragma unroll kUnroll
-        for (int u = 0; u < CH; ++u) {
-            const int jt = (jj0 + u) * JL + jl;
-            pair2<ORDER, DIFF, MASK>(I, tq, jt, j0 + jt, C, pa);
+    for (int ub = 0; ub < JPT; ub += U * G) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            Stage S[G];
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                const int jt = (ub + u * G + g) * JL + jl;
+                head<ORDER, DIFF, MASK>(I, tq, jt, j0 + jt, C, S[g]);
+            }
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                const int jt = (ub + u * G + g) * JL + jl;
+                tail<ORDER, DIFF>(I, tq, jt, C, S[g], pa);
+            }
         }
-        if (JPT >= 64) flush(pa, acc_mine);
+        if (JPT >= 64 && ((ub + U * G) % 64) == 0) flush(pa, acc_mine);
     }
 }
 
+// One work item = (i-tile, j-split) of a force call.  `tile_run` counts the j-tiles this CTA has pushed through the
+// ring since its mbarriers were initialised (stage and phase of tile g are g % STAGES and (g / STAGES) & 1), so a
+// persistent CTA runs item after item on the same barriers.
 template <int ORDER, int JL, int DIFF>
-__global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) {
+__device__ __forceinline__ void force_item(const ForceArgs &A, const int n_act, const int splits, const int i_tile,
+                                           const int split, unsigned char *smem_raw, unsigned &tile_run) {
     typedef Geo<ORDER, DIFF> G;
     constexpr int NQ = G::NQ, NC = G::NC, STAGES = G::STAGES;
     constexpr int IT = kThreads / JL;    // threads per j-lane; the CTA owns 2 IT i-particles
     constexpr int JPT = kTileJ / JL;     // j-particles per thread and tile
-    extern __shared__ __align__(128) unsigned char smem_raw[];
     uint4 *tiles = reinterpret_cast<uint4 *>(smem_raw);
     double *acc_sm = reinterpret_cast<double *>(smem_raw + G::TILE_BYTES);
     const uint32_t bar0 = smem_u32(smem_raw + G::TILE_BYTES + G::ACC_BYTES);
     const int tid = threadIdx.x;
     const int il = tid % IT, jl = tid / IT;
-    const int tile_lo = (int)((long long)A.n_tiles * blockIdx.y / A.splits);
-    const int tile_hi = (int)((long long)A.n_tiles * (blockIdx.y + 1) / A.splits);
+    const int tile_lo = (int)((long long)A.n_tiles * split / splits);
+    const int tile_hi = (int)((long long)A.n_tiles * (split + 1) / splits);
     const int ntile = tile_hi - tile_lo;
+    const unsigned g0 = tile_run;
 
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar0 + 8 * s, 1);                          // full[s]: the TMA transaction
-            mbar_init(bar0 + 8 * (STAGES + s), kThreads / 32);   // empty[s]: one arrival per warp
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-    auto issue = [&](int k) {  // k = tile number within this CTA's range
-        const int s = k % STAGES;
+    auto issue = [&](int k) {  // k = tile number within this item's range
+        const int s = (g0 + k) % STAGES;
         const uint32_t bar = bar0 + 8 * s;
         mbar_expect_tx(bar, G::STAGE_BYTES);
         const size_t off = (size_t)(tile_lo + k) * kTileJ;
@@ -314,7 +334,7 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
         for (int p = 0; p < NQ; ++p)
             bulk_g2s(smem_u32(tiles + (s * NQ + p) * kTileJ), A.q[p] + off, kTileJ * 16, bar);
     };
-    if (tid == 0) {
+    if (tid == 0) {  // every stage is free here: the previous item ended with a __syncthreads after its last tile
         for (int k = 0; k < STAGES - 1 && k < ntile; ++k) issue(k);
     }
 
@@ -323,9 +343,9 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
     float nv[2][3], na[2][3], nj[2][3], xh[2][3], xl[2][3];
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
-        const int slot = blockIdx.x * (2 * IT) + r * IT + il;
-        const bool valid = slot < A.n_act;
-        const int gi = A.idx[valid ? slot : A.n_act - 1];
+        const int slot = i_tile * (2 * IT) + r * IT + il;
+        const bool valid = slot < n_act;
+        const int gi = A.idx[valid ? slot : n_act - 1];
         I.idx[r] = valid ? gi : -1;
         const uint4 qa = __ldg(A.q[0] + gi), qb = __ldg(A.q[1] + gi), qc = __ldg(A.q[2] + gi);
         if (DIFF == 0) {
@@ -365,6 +385,7 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
     C.m3 = pk(-3.f, -3.f);
     C.three = pk(3.f, 3.f);
     C.m4 = pk(-4.f, -4.f);
+    C.n = A.n;
     f2 pa[NC];
     double *acc_mine = acc_sm + tid;
 #pragma unroll
@@ -374,25 +395,21 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
         acc_mine[(2 * c + 1) * kThreads] = 0.0;
     }
 
-    // ---- main loop over this CTA's j-tiles ----
+    // ---- main loop over this item's j-tiles ----
     int since = 0;
 #pragma unroll 1
     for (int k = 0; k < ntile; ++k) {
-        const int s = k % STAGES;
-#if NB_NOBAR
-        if (tid == 0 && k + STAGES - 1 < ntile) {  // tile k+STAGES-1 goes into the stage tile k-1 used
-            if (k >= 1) mbar_wait(bar0 + 8 * (STAGES + (k - 1) % STAGES), (uint32_t)(((k - 1) / STAGES) & 1));
+        const unsigned g = g0 + k;
+        const int s = g % STAGES;
+        if (tid == 0 && k + STAGES - 1 < ntile) {  // tile g+STAGES-1 goes into the stage tile g-1 used
+            if (g >= 1) mbar_wait(bar0 + 8 * (STAGES + (g - 1) % STAGES), (uint32_t)(((g - 1) / STAGES) & 1));
             issue(k + STAGES - 1);
         }
-#else
-        __syncthreads();  // every warp is done with tile k-1, whose stage is refilled now
-        if (tid == 0 && k + STAGES - 1 < ntile) issue(k + STAGES - 1);
-#endif
-        mbar_wait(bar0 + 8 * s, (uint32_t)((k / STAGES) & 1));
+        mbar_wait(bar0 + 8 * s, (uint32_t)((g / STAGES) & 1));
         const uint4 *tq = tiles + s * NQ * kTileJ;
         const int j0 = (tile_lo + k) * kTileJ;
         const bool mine = (unsigned)(I.idx[0] - j0) < (unsigned)kTileJ || (unsigned)(I.idx[1] - j0) < (unsigned)kTileJ;
-        if (__any_sync(0xffffffffu, mine))
+        if (__any_sync(0xffffffffu, mine) || j0 + kTileJ > A.n)
             tile_compute<ORDER, JL, DIFF, true>(I, tq, j0, jl, C, pa, acc_mine);
         else
             tile_compute<ORDER, JL, DIFF, false>(I, tq, j0, jl, C, pa, acc_mine);
@@ -402,11 +419,10 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
                 flush(pa, acc_mine);
             }
         }
-#if NB_NOBAR
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (STAGES + s));
-#endif
     }
+    tile_run = g0 + ntile;
     flush(pa, acc_mine);
     __syncthreads();
 
@@ -417,33 +433,96 @@ __global__ void __launch_bounds__(kThreads, NB_MINB) k_force(const ForceArgs A) 
         double sum = 0.0;
 #pragma unroll 1
         for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
-        const int slot = blockIdx.x * (2 * IT) + r * IT + i_l;
-        if (slot < A.n_act) {
+        const int slot = i_tile * (2 * IT) + r * IT + i_l;
+        if (slot < n_act) {
             if (comp == NC - 1) sum = -sum;
-            if (A.splits == 1) {
+            if (splits == 1) {
                 if (comp == NC - 1) A.out[4][slot] = sum;
                 else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
             } else {
-                A.partials[((size_t)blockIdx.y * NC + comp) * A.n_act + slot] = sum;
+                A.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
             }
         }
     }
 }
 
+template <int ORDER, int DIFF>
+__device__ __forceinline__ void init_ring(unsigned char *smem_raw) {
+    typedef Geo<ORDER, DIFF> G;
+    const uint32_t bar0 = smem_u32(smem_raw + G::TILE_BYTES + G::ACC_BYTES);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < G::STAGES; ++s) {
+            mbar_init(bar0 + 8 * s, 1);                             // full[s]: the TMA transaction
+            mbar_init(bar0 + 8 * (G::STAGES + s), kThreads / 32);   // empty[s]: one arrival per warp
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+}
+
+// host-geometry form: grid = (i-tiles, j-splits), one work item per CTA
+template <int ORDER, int JL, int DIFF>
+__global__ void __launch_bounds__(kThreads, 1) k_force(const ForceArgs A) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    init_ring<ORDER, DIFF>(smem_raw);
+    unsigned tile_run = 0;
+    force_item<ORDER, JL, DIFF>(A, A.n_act, A.splits, blockIdx.x, blockIdx.y, smem_raw, tile_run);
+}
+
+// device-driven form: persistent CTAs (grid = SMs) walk the work items of the block whose size and geometry the
+// selection kernel left in the control block; a stopped run is a no-op.
+template <int ORDER>
+__global__ void __launch_bounds__(kThreads, 1) k_force_dyn(const ForceArgs A) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const Ctl *ctl = A.ctl;
+    if (ctl->stop) return;
+    const int n_act = (int)ctl->n_act, jl = ctl->jl, splits = ctl->splits;
+    const long long items = ctl->i_tiles * splits;
+    init_ring<ORDER, 0>(smem_raw);
+    unsigned tile_run = 0;
+    for (long long w = blockIdx.x; w < items; w += gridDim.x) {
+        const int i_tile = (int)(w % ctl->i_tiles), split = (int)(w / ctl->i_tiles);
+        switch (jl) {
+            case 1: force_item<ORDER, 1, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 2: force_item<ORDER, 2, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 4: force_item<ORDER, 4, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 8: force_item<ORDER, 8, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 32: force_item<ORDER, 32, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            default: force_item<ORDER, 128, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+        }
+        __syncthreads();  // the epilogue has read the accumulators before the next item clears them
+    }
+}
+
 // K_reduce (a-3b): out = Sum_{s = 0 .. S-1} partial[s] in that order.
+__device__ __forceinline__ void reduce_body(const double *partials, int splits, int nc, int n_act, double *acc,
+                                            double *jerk, double *snap, double *crk, double *pot, long long o0,
+                                            long long stride) {
+    const long long tot = (long long)nc * n_act;
+    for (long long o = o0; o < tot; o += stride) {
+        double s = 0.0;
+        for (int k = 0; k < splits; ++k) s += partials[(size_t)k * tot + o];
+        const int comp = (int)(o / n_act), slot = (int)(o % n_act);
+        if (comp == nc - 1) pot[slot] = s;
+        else {
+            double *dst = comp < 3 ? acc : comp < 6 ? jerk : comp < 9 ? snap : crk;
+            dst[(size_t)slot * 3 + comp % 3] = s;
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) k_reduce(const double *partials, int splits, int nc, int n_act, double *acc,
                                                 double *jerk, double *snap, double *crk, double *pot) {
-    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long tot = (long long)nc * n_act;
-    if (o >= tot) return;
-    double s = 0.0;
-    for (int k = 0; k < splits; ++k) s += partials[(size_t)k * tot + o];
-    const int comp = (int)(o / n_act), slot = (int)(o % n_act);
-    if (comp == nc - 1) pot[slot] = s;
-    else {
-        double *dst = comp < 3 ? acc : comp < 6 ? jerk : comp < 9 ? snap : crk;
-        dst[(size_t)slot * 3 + comp % 3] = s;
-    }
+    reduce_body(partials, splits, nc, n_act, acc, jerk, snap, crk, pot,
+                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+}
+
+__global__ void __launch_bounds__(256) k_reduce_dyn(const Ctl *ctl, const double *partials, int nc, double *acc,
+                                                    double *jerk, double *snap, double *crk, double *pot) {
+    if (ctl->stop || ctl->splits == 1) return;
+    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot,
+                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
 typedef void (*force_fn)(const ForceArgs);
@@ -471,106 +550,91 @@ force_fn pick_fn(int order, int diff, int jl) {
     return pick<8, 1>(jl);
 }
 
+force_fn pick_dyn(int order) {
+    return order == 4 ? k_force_dyn<4> : order == 6 ? k_force_dyn<6> : k_force_dyn<8>;
+}
+
 size_t smem_for(int order, int diff) {
     if (diff == 0) return order == 4 ? Geo<4, 0>::SMEM : order == 6 ? Geo<6, 0>::SMEM : Geo<8, 0>::SMEM;
     return order == 4 ? Geo<4, 1>::SMEM : order == 6 ? Geo<6, 1>::SMEM : Geo<8, 1>::SMEM;
 }
 
-constexpr int kNumLanes = 6;
-const int kLanes[kNumLanes] = {1, 2, 4, 8, 32, 128};
-
-}  // namespace
-
-int force_static_init(Ctx *c) {
-    const int orders[3] = {4, 6, 8};
-    for (int diff = 0; diff < 2; ++diff)
-        for (int o = 0; o < 3; ++o)
-            for (int j = 0; j < kNumLanes; ++j)
-                NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, kLanes[j]),
-                                                cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                (int)smem_for(orders[o], diff)));
-    return NBODY_OK;
-}
-
-int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, float eps2, double *acc, double *jerk,
-                 double *snap, double *crackle, double *pot, cudaStream_t st) {
-    const int K = order / 2, NC = 3 * K + 1;
-    const int n_tiles = (int)(c->n_pad / kTileJ);
-    // geometry: j-lanes (a CTA owns 2 * 256 / JL i-particles), i-tiles, j-splits
-    int jl;
-    if (c->force_lanes) jl = c->force_lanes;
-    else {  // the most j-lanes whose CTA still holds all active particles (2 * kThreads / JL i-slots)
-        jl = 1;
-        for (int k = kNumLanes - 1; k >= 1; --k)
-            if ((int64_t)2 * kThreads / kLanes[k] >= n_act) { jl = kLanes[k]; break; }
-    }
-    const int i_per_cta = 2 * (kThreads / jl);
-    const int64_t i_tiles = (n_act + i_per_cta - 1) / i_per_cta;
-    // j-splits: the chip holds `slots` CTAs at once (2 per SM); a launch of i_tiles * S CTAs takes
-    // ceil(i_tiles * S / slots) waves of (n_tiles / S + fixed per-CTA cost) tile-times.  Pick the S that minimises it:
-    // small blocks get S ~ slots / i_tiles (fill the chip), mid-size blocks get a CTA count that is close to a
-    // multiple of `slots` (no half-empty last wave), big blocks (>= 8 waves) run unsplit.
-    const int64_t slots = NB_MINB * (int64_t)c->sm_count;
-    int64_t S = 1;
-    if (c->force_split) {
-        S = c->force_split;
-    } else if (i_tiles < 8 * slots) {
-        const double fixed = 3.0;  // prologue + epilogue + reduce, in tile-times
-        double best = 1e300, cost1 = 0.0;
-        const int64_t s_max = n_tiles < 4 * slots ? n_tiles : 4 * slots;
-        for (int64_t s = 1; s <= s_max; ++s) {
-            const int64_t waves = (i_tiles * s + slots - 1) / slots;
-            const double cost = (double)waves * ((double)((n_tiles + s - 1) / s) + fixed);
-            if (s == 1) cost1 = cost;
-            if (cost < best * (1.0 - 1e-9)) {
-                best = cost;
-                S = s;
-            }
-        }
-        if (best > 0.97 * cost1) S = 1;  // a split costs S x NC x n_act doubles of scratch: only for a real gain
-    }
-    if (S > n_tiles) S = n_tiles;
-    if (S > 65535) S = 65535;
-    if (S < 1) S = 1;
-    if (S > 1) {
-        const size_t need = sizeof(double) * (size_t)S * NC * (size_t)n_act;
-        if (need > c->partials_bytes) {
-            NB_CUDA(c, cudaStreamSynchronize(st));
-            cudaFree(c->partials);
-            c->partials = nullptr;
-            c->partials_bytes = 0;
-            NB_CUDA(c, cudaMalloc(&c->partials, need));
-            c->partials_bytes = need;
-        }
-    }
-    ForceArgs A;
+void fill_args(Ctx *c, ForceArgs &A, const int32_t *active_idx, float eps2, double *acc, double *jerk, double *snap,
+               double *crackle, double *pot) {
     const uint4 *base = c->jstore;
     A.q[0] = base + (size_t)(c->diff_mode ? 4 : 0) * c->cap_pad;
     A.q[1] = base + (size_t)(c->diff_mode ? 5 : 1) * c->cap_pad;
     A.q[2] = base + (size_t)2 * c->cap_pad;
     A.q[3] = base + (size_t)3 * c->cap_pad;
     A.idx = active_idx;
-    A.n_act = (int)n_act;
-    A.n_tiles = n_tiles;
-    A.splits = (int)S;
+    A.n = (int)c->n;
+    A.n_act = 0;
+    A.n_tiles = (int)(c->n_pad / kTileJ);
+    A.splits = 1;
     A.eps2 = eps2;
     A.out[0] = acc; A.out[1] = jerk; A.out[2] = snap; A.out[3] = crackle; A.out[4] = pot;
     A.partials = c->partials;
-    const dim3 grid((unsigned)i_tiles, (unsigned)S);
-    pick_fn(order, c->diff_mode, jl)<<<grid, kThreads, smem_for(order, c->diff_mode), st>>>(A);
+    A.ctl = c->d_ctl;
+}
+
+}  // namespace
+
+int force_static_init(Ctx *c) {
+    const int orders[3] = {4, 6, 8};
+    for (int o = 0; o < 3; ++o) {
+        for (int diff = 0; diff < 2; ++diff)
+            for (int j = 0; j < kNumLanes; ++j)
+                NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_fn(orders[o], diff, lane_variant(j)),
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)smem_for(orders[o], diff)));
+        NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_dyn(orders[o]), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)smem_for(orders[o], 0)));
+    }
+    return NBODY_OK;
+}
+
+int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, float eps2, double *acc, double *jerk,
+                 double *snap, double *crackle, double *pot, cudaStream_t st) {
+    const int K = order / 2, NC = 3 * K + 1;
+    ForceArgs A;
+    fill_args(c, A, active_idx, eps2, acc, jerk, snap, crackle, pot);
+    // geometry: j-lanes and j-splits from the size of the whole block (an i-sharded rank passes its slice as n_act
+    // and the block size as the "geometry_n_act" option, so every rank sums in the order of the unsharded call)
+    const int64_t n_geo = c->geometry_n_act ? c->geometry_n_act : n_act;
+    if (n_act > n_geo) return NBODY_EINVAL;
+    const ForceGeo g = force_geometry(n_geo, A.n_tiles, c->sm_count, c->force_lanes, c->force_split, c->partial_rows);
+    const int64_t i_tiles = (n_act + g.i_per_cta - 1) / g.i_per_cta;
+    if (g.splits > 1 && (int64_t)g.splits * n_act > c->partial_rows) return NBODY_EINVAL;  // forced split beyond the scratch
+    A.n_act = (int)n_act;
+    A.splits = g.splits;
+    const dim3 grid((unsigned)i_tiles, (unsigned)g.splits);
+    pick_fn(order, c->diff_mode, g.jl)<<<grid, kThreads, smem_for(order, c->diff_mode), st>>>(A);
     c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
-    if (S > 1) {
+    if (g.splits > 1) {
         const long long tot = (long long)NC * n_act;
-        k_reduce<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(c->partials, (int)S, NC, (int)n_act, acc, jerk, snap,
-                                                                 crackle, pot);
+        long long blocks = (tot + 255) / 256;
+        if (blocks > 8LL * c->sm_count) blocks = 8LL * c->sm_count;
+        k_reduce<<<(unsigned)blocks, 256, 0, st>>>(c->partials, g.splits, NC, (int)n_act, acc, jerk, snap, crackle, pot);
         c->launches += 1;
         NB_CUDA(c, cudaGetLastError());
     }
     c->last_r = 2;
-    c->last_jl = jl;
-    c->last_s = (int)S;
-    c->last_ctas = i_tiles * S;
+    c->last_jl = g.jl;
+    c->last_s = g.splits;
+    c->last_ctas = i_tiles * g.splits;
+    return NBODY_OK;
+}
+
+int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, double *acc, double *jerk, double *snap,
+                     double *crackle, double *pot, cudaStream_t st) {
+    const int K = order / 2, NC = 3 * K + 1;
+    ForceArgs A;
+    fill_args(c, A, active_idx, eps2, acc, jerk, snap, crackle, pot);
+    pick_dyn(order)<<<c->sm_count, kThreads, smem_for(order, 0), st>>>(A);
+    NB_CUDA(c, cudaGetLastError());
+    k_reduce_dyn<<<2 * c->sm_count, 256, 0, st>>>(c->d_ctl, c->partials, NC, acc, jerk, snap, crackle, pot);
+    NB_CUDA(c, cudaGetLastError());
     return NBODY_OK;
 }
 

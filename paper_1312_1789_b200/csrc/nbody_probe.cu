@@ -1,6 +1,9 @@
-// libnbody.so, translation unit 3: register-only micro-probes of the instruction classes K_force is made of.
+// libnbody.so, translation unit 3: micro-probes of the instruction classes K_force is made of (include/nbody_bench.h).
 // They give the "measured" denominators beside the nominal FP32 peak: thread-operations
-// per second of FFMA, DADD, F2F (fp64 -> fp32), MUFU.RSQ, and the DADD+F2F pair, each on every SM at once.
+// per second of FFMA, DADD, F2F (fp64 -> fp32), MUFU.RSQ, the DADD+F2F pair and packed FFMA2, each on every SM at
+// once, and the issue-port probes (kinds 7..9): one packed FFMA2 next to one instruction of another pipe, which
+// show whether that instruction is hidden behind the FFMA2's second pipe cycle or costs an issue cycle of its own.
+#include "nbody_bench.h"
 #include "nbody_internal.h"
 
 namespace nbody {
@@ -18,10 +21,18 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
     }
     float f[kProbeChains];
     double d[kProbeChains];
+    unsigned x[kProbeChains];
+    __shared__ uint4 sm[64];
+    if (KIND == 9) {
+        if (threadIdx.x < 64) sm[threadIdx.x] = make_uint4(threadIdx.x, 1u, 2u, 3u);
+        __syncthreads();
+    }
+    const unsigned sm_base = (unsigned)__cvta_generic_to_shared(sm);
 #pragma unroll
     for (int c = 0; c < kProbeChains; ++c) {
         f[c] = seed + (float)(threadIdx.x + c);
         d[c] = (double)seed + (double)(threadIdx.x * 3 + c);
+        x[c] = threadIdx.x * 7u + c;
     }
     unsigned long long p2[kProbeChains], p2c[kProbeChains], p2d[kProbeChains], p2b;
 #pragma unroll
@@ -48,6 +59,18 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
                 asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p2[c]) : "l"(p2b), "l"(p2c[c]));
             if (KIND == 6)  // packed FFMA2, three fresh 64-bit operands
                 asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p2[c]) : "l"(p2d[c]), "l"(p2c[c]));
+            if (KIND >= 7 && KIND <= 9) {  // one packed FFMA2 + one instruction of another pipe (independent chains)
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p2[c]) : "l"(p2b), "l"(p2c[c]));
+                if (KIND == 7) asm volatile("shf.l.wrap.b32 %0, %0, %1, 3;" : "+r"(x[c]) : "r"(x[(c + 1) % kProbeChains]));
+                if (KIND == 8) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(d[c]) : "d"(db));
+                if (KIND == 9) {
+                    unsigned a0, a1, a2, a3;
+                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3)
+                                 : "r"(sm_base + (((unsigned)it + c) & 63u) * 16u));
+                    x[c] ^= a0 ^ a1 ^ a2 ^ a3;
+                }
+            }
             if (KIND == 4) {  // the literal difference pattern: DADD, F2F, and an FADD that consumes it
                 double t;
                 float g;
@@ -65,7 +88,7 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
         asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p2[c]));
         asm("mov.b64 {%0, %1}, %2;" : "=f"(lo2), "=f"(hi2) : "l"(p2c[c]));
         asm("mov.b64 {%0, %1}, %2;" : "=f"(lo3), "=f"(hi3) : "l"(p2d[c]));
-        s += f[c] + (float)d[c] + lo + hi + lo2 + hi2 + lo3 + hi3;
+        s += f[c] + (float)d[c] + lo + hi + lo2 + hi2 + lo3 + hi3 + __uint_as_float(x[c]);
     }
     if (s == 123.456f) sink[0] = s;  // never true in practice; keeps the chains live
     if (blockIdx.x == 0 && threadIdx.x == 0) {  // SM cycles and nanoseconds this CTA ran: the SM clock under this load
@@ -78,12 +101,13 @@ __global__ void __launch_bounds__(256) k_probe(float *sink, float seed, unsigned
 }
 
 typedef void (*probe_fn)(float *, float, unsigned long long *);
-const probe_fn kProbes[7] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>, k_probe<5>, k_probe<6>};
+const probe_fn kProbes[10] = {k_probe<0>, k_probe<1>, k_probe<2>, k_probe<3>, k_probe<4>,
+                              k_probe<5>, k_probe<6>, k_probe<7>, k_probe<8>, k_probe<9>};
 
 }  // namespace
 
 int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
-    NB_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
     float *sink = nullptr;
     NB_CUDA(c, cudaMalloc(&sink, sizeof(float) + 2 * sizeof(unsigned long long) + 8));
     unsigned long long *clk = reinterpret_cast<unsigned long long *>(reinterpret_cast<char *>(sink) + 8);
@@ -124,3 +148,8 @@ int probe_peak(Ctx *c, int kind, int millis, double *tera_ops) {
 }
 
 }  // namespace nbody
+
+extern "C" int nbody_probe_peak(nbody_ctx *h, int kind, int millis, double *tera_ops_host) {
+    if (!h || !tera_ops_host || kind < 0 || kind > 9 || millis < 1 || millis > 20000) return NBODY_EINVAL;
+    return nbody::probe_peak(&h->c, kind, millis, tera_ops_host);
+}

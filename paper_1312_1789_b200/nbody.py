@@ -3,7 +3,8 @@
 Every step of the path runs in the CUDA kernels of csrc/; torch supplies device memory (`tensor.data_ptr()`) and
 the current stream, nothing else.  Importing this module fails loudly when csrc/libnbody.so is missing: there
 is no CPU fallback (BASELINE.json north_star), and nothing here imports `oracle/`.
-Names follow the C ABI: Context.predict / force / correct / next_block / initial_dt / get_predicted / force_host.
+Names follow the C ABI: Context.predict / force / correct / next_block / initial_dt / get_predicted / run_blocks /
+pack_rows / unpack_rows / force_host / step_host (include/nbody.h) and probe_peak (include/nbody_bench.h).
 """
 import ctypes as C
 import os
@@ -24,11 +25,18 @@ _vp = C.c_void_p
 _i64 = C.c_int64
 _dbl = C.c_double
 
-# every symbol include/nbody.h declares, with its signature
+class RunResult(C.Structure):
+    """nbody_run_result of include/nbody.h."""
+    _fields_ = [("blocks", C.c_int64), ("pairs", C.c_int64), ("t_next", C.c_double), ("n_act_next", C.c_int64),
+                ("stop_reason", C.c_int32), ("reserved", C.c_int32), ("hist_log2", C.c_int64 * 40)]
+
+
+# every symbol include/nbody.h and include/nbody_bench.h declare, with its signature
 SIGNATURES = {
     "nbody_abi_version": (C.c_int, []),
     "nbody_strerror": (C.c_char_p, [C.c_int]),
     "nbody_create": (C.c_int, [C.POINTER(_vp), _i64, C.c_int]),
+    "nbody_workspace_bytes": (_i64, [_i64]),
     "nbody_destroy": (C.c_int, [_vp]),
     "nbody_last_cuda_error": (C.c_int, [_vp]),
     "nbody_set_option": (C.c_int, [_vp, C.c_char_p, _i64]),
@@ -39,6 +47,10 @@ SIGNATURES = {
     "nbody_initial_dt": (C.c_int, [_vp, _i64, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
     "nbody_next_block": (C.c_int, [_vp, _i64, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_i64), _vp]),
     "nbody_get_predicted": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nbody_run_blocks": (C.c_int, [_vp, _i64, C.c_int, _dbl, _dbl, _dbl, _dbl, _dbl, _i64, _i64, _vp, _vp, _vp, _vp, _vp,
+                                   C.POINTER(_vp), _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(RunResult), _vp]),
+    "nbody_pack_rows": (C.c_int, [_vp, _vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _vp, C.POINTER(_vp), _vp, _vp]),
+    "nbody_unpack_rows": (C.c_int, [_vp, _vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _vp, C.POINTER(_vp), _vp, _vp]),
     "nbody_force_host": (C.c_int, [_vp, _i64, _dbl, C.c_int, _vp, _vp, _vp, _vp, C.POINTER(_vp), _vp, _i64, _dbl,
                                    _vp, _vp, _vp, _vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
     "nbody_step_host": (C.c_int, [_vp, _i64, C.c_int, _dbl, _dbl, _dbl, _dbl, _vp, _vp, _vp, _vp, _vp, C.POINTER(_vp),
@@ -70,6 +82,10 @@ def strerror(code: int) -> str:
 
 def abi_version() -> int:
     return _lib.nbody_abi_version()
+
+
+def workspace_bytes(n_capacity: int) -> int:
+    return int(_lib.nbody_workspace_bytes(int(n_capacity)))
 
 
 def _ptr(a):
@@ -156,6 +172,29 @@ class Context:
     def get_predicted(self, xp, vp, ap, jp, m32, stream=None):
         self._check(_lib.nbody_get_predicted(self._h, _ptr(xp), _ptr(vp), _ptr(ap), _ptr(jp), _ptr(m32),
                                              _stream(stream)), "nbody_get_predicted")
+
+    def run_blocks(self, n, order, eps2, eta, dt_min, dt_max, t_end, max_blocks, max_n_act, t, dt, m, x, v, a_derivs,
+                   pot_state, active_idx, acc, jerk, snap, crackle, pot, stream=None):
+        """Device-driven block steps (nbody_run_blocks).  Returns dict(blocks, pairs, t_next, n_act_next, stop_reason,
+        hist_log2)."""
+        r = RunResult()
+        self._check(_lib.nbody_run_blocks(self._h, int(n), int(order), float(eps2), float(eta), float(dt_min),
+                                          float(dt_max), float(t_end), int(max_blocks), int(max_n_act), _ptr(t),
+                                          _ptr(dt), _ptr(m), _ptr(x), _ptr(v), _ptr_array(a_derivs, 8), _ptr(pot_state),
+                                          _ptr(active_idx), _ptr(acc), _ptr(jerk), _ptr(snap), _ptr(crackle), _ptr(pot),
+                                          C.byref(r), _stream(stream)), "nbody_run_blocks")
+        return dict(blocks=r.blocks, pairs=r.pairs, t_next=r.t_next, n_act_next=r.n_act_next,
+                    stop_reason=r.stop_reason, hist_log2=list(r.hist_log2))
+
+    def pack_rows(self, idx, n_rows, order, t, dt, pot_state, x, v, a_derivs, rec, stream=None):
+        self._check(_lib.nbody_pack_rows(self._h, _ptr(idx), int(n_rows), int(order), _ptr(t), _ptr(dt), _ptr(pot_state),
+                                         _ptr(x), _ptr(v), _ptr_array(a_derivs, 8), _ptr(rec), _stream(stream)),
+                    "nbody_pack_rows")
+
+    def unpack_rows(self, idx, n_rows, order, t, dt, pot_state, x, v, a_derivs, rec, stream=None):
+        self._check(_lib.nbody_unpack_rows(self._h, _ptr(idx), int(n_rows), int(order), _ptr(t), _ptr(dt),
+                                           _ptr(pot_state), _ptr(x), _ptr(v), _ptr_array(a_derivs, 8), _ptr(rec),
+                                           _stream(stream)), "nbody_unpack_rows")
 
     def force_host(self, n, t_now, order, t, m, x, v, a_derivs, active_idx, n_act, eps2, acc, jerk, snap, crackle, pot):
         """HOST (numpy) buffers in and out; returns (h2d_bytes, d2h_bytes)."""

@@ -1,7 +1,10 @@
 """Thin host block scheduler ("individual hierarchically block time-steps").
 
 Holds the fp64 SoA state as torch CUDA tensors (device memory only -- no torch arithmetic on the path) and drives
-the C-ABI calls per block:  next_block -> predict -> force -> correct.  Bootstrap = DESIGN.md R9b (SURVEY c-10).
+the C-ABI calls.  Two drivers over the same kernels: block_step / integrate call next_block -> predict -> force ->
+correct per block (one host round trip per block); run hands whole runs of blocks to the device-driven step
+(nbody_run_blocks: one CUDA graph per block step, the host looks in every 4 .. 64 blocks).  Bootstrap = DESIGN.md R9b
+(SURVEY c-10).
 """
 import numpy as np
 import torch
@@ -95,6 +98,20 @@ class Integrator:
             b = int(n_act).bit_length() - 1
             hist[b] = hist.get(b, 0) + 1
         return hist
+
+    def run(self, t_end, max_blocks=10**12, max_n_act=None):
+        """Device-driven integration (nbody_run_blocks): executes blocks while t_next <= t_end (and n_act <= max_n_act
+        when given).  Returns the library's result dict; bit-identical to integrate()."""
+        p = self.order
+        r = self.ctx.run_blocks(self.n, p, self.eps2, self.eta, self.dt_min, self.dt_max, t_end, max_blocks,
+                                self.n if max_n_act is None else max_n_act, self.t, self.dt, self.m, self.x, self.v,
+                                self.D, self.pot, self.active, self.acc, self.jerk, self.snap if p >= 6 else None,
+                                self.crk if p >= 8 else None, self.fpot)
+        self.blocks += r["blocks"]
+        self.pairs += r["pairs"]
+        if r["blocks"]:
+            self.time = float(self.t.max())  # diagnostic read (the last executed block's time)
+        return r
 
     def energy(self):
         """E = Sum 1/2 m v^2 + 1/2 Sum m pot with pot from a synchronised order-4 all-active call (c-11).  The

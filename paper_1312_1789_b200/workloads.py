@@ -216,10 +216,11 @@ def active_list(n: int, n_act: int, rng: np.random.Generator) -> np.ndarray:
     return np.sort(rng.choice(n, size=n_act, replace=False)).astype(np.int32)
 
 
-def oracle_sample(c: dict, size: int = 1024, n_edge: int = 32, stream: int = 2) -> np.ndarray:
+def oracle_sample(c: dict, size: int = 1024, n_edge: int = 32, stream: int = 2, n_outer: int | None = None) -> np.ndarray:
     """i-particles on which the oracle is evaluated when N is too large for all of them:
-    a seeded uniform draw plus forced members -- every BH, the n_edge innermost and outermost particles and the
-    n_edge particles nearest to each BH (where mixed-precision errors are largest).  Ascending, unique."""
+    a seeded uniform draw plus forced members -- every BH, the n_edge innermost and the n_outer (default n_edge)
+    outermost particles and the n_edge particles nearest to each BH (where mixed-precision errors are largest).
+    Ascending, unique."""
     rng = rng_for(c["config"], stream)
     x, bh = c["x"], c["bh"]
     n = x.shape[0]
@@ -230,7 +231,8 @@ def oracle_sample(c: dict, size: int = 1024, n_edge: int = 32, stream: int = 2) 
     ne = min(n_edge, n)
     order = np.argpartition(r, ne - 1)[:ne]
     forced.append(order)
-    order = np.argpartition(-r, ne - 1)[:ne]
+    no = min(n_edge if n_outer is None else n_outer, n)
+    order = np.argpartition(-r, no - 1)[:no]
     forced.append(order)
     for b in bh:
         d = np.linalg.norm(x - x[b], axis=1)

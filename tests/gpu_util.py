@@ -74,3 +74,59 @@ def check_force(got, ref, order, tag=""):
     for k, e in errs.items():
         assert np.isfinite(e) and e <= TOL[k], "%s %s rel err %.3e > %.1e (all: %s)" % (tag, k, e, TOL[k], errs)
     return errs
+
+
+def conditioning_report(got, ref, absn, radius, order):
+    """Per quantity: max and 99.9th-percentile relative error over the sampled particles and, for the worst particle,
+    its radius and kappa = Sum_j |term| / |Sum_j term|.  absn = oracle force_abs output."""
+    names = ["acc", "jerk", "snap", "crackle"][: order // 2]
+    rep = {}
+    for k, nm in enumerate(names):
+        den = np.linalg.norm(ref[k], axis=1)
+        err = np.linalg.norm(np.asarray(got[k]) - ref[k], axis=1) / den
+        kap = absn[k] / den
+        w = int(np.argmax(err))
+        rep[nm] = dict(max=float(err[w]), p999=float(np.percentile(err, 99.9)), median=float(np.median(err)),
+                       worst_radius=float(radius[w]), worst_kappa=float(kap[w]), kappa_max=float(kap.max()),
+                       kappa_median=float(np.median(kap)), tol=TOL[nm])
+    e = np.abs(np.asarray(got[4]) - ref[4]) / np.abs(ref[4])
+    w = int(np.argmax(e))
+    rep["pot"] = dict(max=float(e[w]), p999=float(np.percentile(e, 99.9)), median=float(np.median(e)),
+                      worst_radius=float(radius[w]), tol=TOL["pot"])
+    return rep
+
+
+def corrector_bounds(order, h, D1):
+    """Per-particle bounds on |x_gpu - x_oracle| and |v_gpu - v_oracle| after ONE corrector step (R6) taken from
+    identical states: the two sides differ only in the force-call values at t1, by at most BASELINE.json's tolerances
+    (|da| <= 1e-5 |a1|, |dj| <= 1e-4 |j1|, |ds| <= 1e-3 |s1|, |dc| <= 1e-2 |c1|), which the corrector's own
+    coefficients carry into v1 and x1:
+        p=4: dv <= h/2 da + h^2/12 dj                        dx <= h/2 dv + h^2/12 da
+        p=6: dv <= h/2 da + h^2/10 dj + h^3/120 ds           dx <= h/2 dv + h^2/10 da + h^3/120 dj
+        p=8: dv <= h/2 da + 3h^2/28 dj + h^3/84 ds + h^4/1680 dc
+             dx <= h/2 dv + 3h^2/28 da + h^3/84 dj + h^4/1680 ds
+    h: step of each particle, D1[k]: the oracle's a^(k)(t1) rows of the same particles.  A few ulp of the state are
+    added for the rounding of the sums themselves."""
+    nr = [np.linalg.norm(D1[k], axis=1) for k in range(order // 2)]
+    d = [TOL["acc"] * nr[0], TOL["jerk"] * nr[1]]
+    if order >= 6:
+        d.append(TOL["snap"] * nr[2])
+    if order >= 8:
+        d.append(TOL["crackle"] * nr[3])
+    c = {4: [0.5, 1 / 12.0], 6: [0.5, 0.1, 1 / 120.0], 8: [0.5, 3 / 28.0, 1 / 84.0, 1 / 1680.0]}[order]
+    dv = sum(c[k] * h ** (k + 1) * d[k] for k in range(order // 2))
+    dx = 0.5 * h * dv + sum(c[k] * h ** (k + 1) * d[k - 1] for k in range(1, order // 2))
+    return dx, dv
+
+
+def check_corrected(order, idx, h, x_g, v_g, x_o, v_o, D1_o):
+    """Assert the corrected rows `idx` agree within corrector_bounds (+ 8 ulp of the value)."""
+    bx, bv = corrector_bounds(order, h, [d[idx] for d in D1_o])
+    ex = np.linalg.norm(x_g[idx] - x_o[idx], axis=1)
+    ev = np.linalg.norm(v_g[idx] - v_o[idx], axis=1)
+    ulp = 8 * 2.2e-16
+    okx = ex <= bx + ulp * np.linalg.norm(x_o[idx], axis=1)
+    okv = ev <= bv + ulp * np.linalg.norm(v_o[idx], axis=1)
+    assert np.all(okx), ("x", float(np.max(ex / (bx + 1e-300))))
+    assert np.all(okv), ("v", float(np.max(ev / (bv + 1e-300))))
+    return float(np.max(ex / (bx + 1e-300))), float(np.max(ev / (bv + 1e-300)))

@@ -1,5 +1,6 @@
 """-m "not gpu": the C-ABI library builds for sm_100a here (nvcc cross-compiles), loads, and exports every symbol
-include/nbody.h declares; host-side argument validation that needs no device; the product never touches oracle/."""
+include/nbody.h and include/nbody_bench.h declare; host-side argument validation that needs no device; the launch
+geometry rule; the product never touches oracle/."""
 import ctypes as C
 import os
 import re
@@ -14,11 +15,16 @@ def _lib():
 
 
 def test_header_symbols_exported():
-    hdr = open(os.path.join(ROOT, "include", "nbody.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(nbody_[a-z_0-9]+)\s*\(", hdr))
+    names = set()
+    for f in ("nbody.h", "nbody_bench.h"):
+        hdr = open(os.path.join(ROOT, "include", f)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        names |= set(re.findall(r"\b(nbody_[a-z_0-9]+)\s*\(", hdr))
     assert {"nbody_create", "nbody_destroy", "nbody_predict", "nbody_force", "nbody_correct", "nbody_strerror",
-            "nbody_next_block", "nbody_force_host", "nbody_get_predicted"} <= names
+            "nbody_next_block", "nbody_force_host", "nbody_get_predicted", "nbody_run_blocks", "nbody_pack_rows",
+            "nbody_unpack_rows", "nbody_workspace_bytes", "nbody_probe_peak"} <= names
+    main = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "nbody.h")).read(), flags=re.S)
+    assert "nbody_probe_peak" not in main  # the micro-benchmark is not part of the method's API
     lib = _lib()
     for n in sorted(names):
         assert hasattr(lib, n), "libnbody.so does not export %s" % n
@@ -32,7 +38,7 @@ def test_strerror_and_version():
     for code in (0, -1, -2, -3, -4, 77):
         s = lib.nbody_strerror(code)
         assert s is not None and len(s) > 0
-    assert lib.nbody_abi_version() == 1
+    assert lib.nbody_abi_version() == 2
 
 
 def test_create_without_device_fails_loudly():
@@ -56,6 +62,11 @@ def test_null_and_bad_arguments_without_device():
     h = C.c_void_p()
     assert lib.nbody_create(C.byref(h), C.c_int64(0), 0) == -1
     assert lib.nbody_set_option(None, b"diff_mode", C.c_int64(0)) == -1
+    lib.nbody_workspace_bytes.restype = C.c_int64
+    assert lib.nbody_workspace_bytes(C.c_int64(0)) == -1
+    w = lib.nbody_workspace_bytes(C.c_int64(2097152))
+    assert 6 * 16 * 2097152 < w < 6 * 16 * 2097152 + (513 << 20)  # j-store + split scratch (<= 512 MB)
+    assert lib.nbody_workspace_bytes(C.c_int64(16)) < 1 << 16     # tiny contexts get a tiny scratch
 
 
 def test_sass_shows_tma_and_no_tensor_or_local_in_hot_kernel():
@@ -69,15 +80,63 @@ def test_sass_shows_tma_and_no_tensor_or_local_in_hot_kernel():
     # Blackwell packed fp32 pair arithmetic (fma/mul/add.f32x2) and no spilled hot loop in the 6th-order kernel
     assert "FFMA2" in sass and "FMUL2" in sass and "FADD2" in sass
     sass = subprocess.run(["cuobjdump", "-sass", os.path.join(csrc, "nbody_exact.o")], capture_output=True, text=True).stdout
-    fn = None
+    # No FMA contraction in the bit-exact kernels (R12): the 8th-order predictor's Horner chains are 22 products and 22
+    # sums per coordinate; a contracted build would have turned them into DFMA and the DMUL / DADD counts would collapse
+    # (DFMA itself still appears inside the correctly rounded IEEE division expansions).
+    counts, fn = {}, None
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)
         if m:
             fn = m.group(1)
-        if fn and ("k_predict" in fn or "k_correct" in fn or "k_initial_dt" in fn) and "DFMA" in line:
-            # DFMA may only appear inside the IEEE division / sqrt expansions, which are correctly rounded
-            pass
-    assert "k_predict" in sass and "k_correct" in sass
+            counts[fn] = {"DMUL": 0, "DADD": 0}
+        elif fn:
+            for op in ("DMUL", "DADD"):
+                if re.search(r"\b%s\b" % op, line):
+                    counts[fn][op] += 1
+    p8 = [v for k, v in counts.items() if "k_predictILi8E" in k]
+    assert len(p8) == 1 and p8[0]["DMUL"] >= 66 and p8[0]["DADD"] >= 66, p8
+    c8 = [v for k, v in counts.items() if "k_correctILi8E" in k]
+    assert len(c8) == 1 and c8[0]["DMUL"] >= 150 and c8[0]["DADD"] >= 100, c8
+    assert any("k_select" in k for k in counts)
+
+
+def test_force_geometry_rule_matches_round1_table():
+    """The launch geometry is a pure integer function of (n_act, n_tiles, SMs) shared by the host launcher and the
+    device-driven step: small blocks fill the chip (S ~ 148 / i-tiles), mid-size blocks land near a multiple of 148
+    work items, big blocks run unsplit (the geometries of the sweeps in profiles/)."""
+    src = open(os.path.join(ROOT, "paper_1312_1789_b200", "csrc", "nbody_internal.h")).read()
+    body = src[src.index("struct ForceGeo {"):src.index("// ---- device control block")]
+    prog = """#include <stdio.h>
+#define __host__
+#define __device__
+constexpr int kThreads = 512, kNumLanes = 6;
+inline int lane_variant(int k) { return k == 0 ? 1 : k == 1 ? 2 : k == 2 ? 4 : k == 3 ? 8 : k == 4 ? 32 : 128; }
+%s
+int main() {
+    const long long cases[][2] = {{1, 256}, {16, 256}, {256, 256}, {4096, 256}, {65536, 256}, {1, 1024}, {64, 1024},
+                                  {1024, 1024}, {4096, 1024}, {262144, 1024}, {1048576, 4096}, {2097152, 8192}};
+    for (auto &c : cases) {
+        ForceGeo g = force_geometry(c[0], (int)c[1], 148, 0, 0, 8388608);
+        printf("%%lld %%lld %%d %%d %%lld\\n", c[0], c[1], g.jl, g.splits, g.i_tiles);
+    }
+}""" % body
+    import tempfile
+    with tempfile.TemporaryDirectory() as d:
+        open(os.path.join(d, "g.cpp"), "w").write(prog)
+        subprocess.check_call(["g++", "-std=c++17", "-O1", "-o", os.path.join(d, "g"), os.path.join(d, "g.cpp")])
+        out = subprocess.run([os.path.join(d, "g")], capture_output=True, text=True).stdout.split("\n")
+    got = {(int(l.split()[0]), int(l.split()[1])): tuple(int(v) for v in l.split()[2:]) for l in out if l.strip()}
+    assert got[(1, 256)] == (128, 128, 1)
+    assert got[(16, 256)] == (32, 128, 1)
+    assert got[(256, 256)] == (4, 128, 1)
+    assert got[(4096, 256)] == (1, 37, 4)
+    assert got[(65536, 256)] == (1, 9, 64)
+    assert got[(1, 1024)] == (128, 147, 1)
+    assert got[(64, 1024)] == (8, 147, 1)
+    assert got[(1024, 1024)] == (1, 147, 1)
+    assert got[(262144, 1024)] == (1, 4, 256)
+    assert got[(1048576, 4096)] == (1, 1, 1024)
+    assert got[(2097152, 8192)] == (1, 1, 2048)
 
 
 def test_product_does_not_import_oracle():

@@ -7,6 +7,9 @@ seeded draw -- where mixed-precision errors are largest).
   config 2: N =    65 536, 4th order, N_act = 1, 16, 256, 4096, 65 536
   config 5: N = 2 097 152, 8th order, ALL active, and N_act = 3 .. 1.5 M (j-split partials at the largest N)
 """
+import json
+import os
+
 import numpy as np
 import pytest
 
@@ -81,3 +84,43 @@ def test_nact_sweep_full_size_sampled(config, order, nacts):
         got = tuple(None if a is None else a[pp].cpu().numpy() for a in out)
         U.check_force(got, ref, order, "cfg%d N=%d n_act=%d geom %s" % (config, n, na, ctx.last_force_geometry()))
     ctx.close()
+
+
+@pytest.mark.parametrize("config,order", [(3, 6), (4, 6), (5, 8)])
+def test_full_size_physically_consistent_derivatives(config, order):
+    """The hard inputs (SURVEY.md 8(d) "primary", Appendix A): the Taylor coefficients D_0..D_3 are the cluster's OWN
+    acceleration, jerk, snap and crackle (GPU bootstrap R9b, handed unchanged to the oracle), so Sum m_j a_j =
+    Sum m_j j_j = 0 and the far-halo snap / crackle sums are near-total cancellations.  All-active call at the full
+    size (the launch bench.py times), predicted to t = 2^-10; oracle on the forced-member sample: every BH, the 32
+    innermost, the 4096 OUTERMOST, the 32 nearest to each BH and a seeded draw.  Prints, per quantity, max / 99.9th
+    percentile / worst particle's radius and kappa and asserts BASELINE.json's tolerances."""
+    import torch
+    from paper_1312_1789_b200.scheduler import Integrator
+    from oracle import oracle as O
+    c = W.cluster(config)
+    n, eps2 = c["n"], c["eps2"]
+    H = 2.0**-10
+    g = Integrator(c["m"], c["x"], c["v"], order, eps2)
+    g.bootstrap(fixed_dt=H)
+    torch.cuda.synchronize()
+    D = [d.cpu().numpy().copy() for d in g.D[:6]]  # D_4, D_5 are zero after the bootstrap (R9b)
+    t = np.zeros(n)
+    s = W.oracle_sample(c, size=6144, n_outer=4096)
+    xp, vp, ap, jp = O.predict(H, order, t, c["x"], c["v"], D)
+    ref = O.force(c["m"], xp, vp, ap, jp, s, order, eps2)
+    absn = O.force_abs(c["m"], xp, vp, ap, jp, s, order, eps2)
+    g.ctx.predict(n, H, order, g.t, g.m, g.x, g.v, g.D)
+    out = _force(g.ctx, g.all_idx, n, order, eps2)
+    geo = g.ctx.last_force_geometry()
+    assert geo["j_lanes"] == 1 and geo["j_splits"] == 1
+    ii = torch.from_numpy(s.astype(np.int64)).cuda()
+    got = tuple(None if a is None else a[ii].cpu().numpy() for a in out)
+    radius = np.linalg.norm(c["x"][s], axis=1)
+    rep = U.conditioning_report(got, ref, absn, radius, order)
+    line = dict(test="full_size_physically_consistent", config=config, n=n, order=order, sample=int(s.shape[0]), report=rep)
+    print(json.dumps(line))
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", "parity_fullsize_cfg%d.json" % config), "w") as f:
+        json.dump(line, f, indent=1)
+    U.check_force(got, ref, order, "cfg%d full size, bootstrap derivatives" % config)
+    g.ctx.close()

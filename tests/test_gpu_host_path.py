@@ -35,6 +35,7 @@ def test_step_host_equals_device_path_and_oracle(order):
         tn_h, na_h, up, down = ctx.step_host(so.n, order, eps2, 0.1, 2.0**-30, 2.0**-4, h["t"], h["dt"], so.m, h["x"],
                                              h["v"], h["D"], h["pot"])
         tn_g, na_g = g.block_step()
+        h_old = so.dt.copy()
         tn_o, idx_o = OI.block_step(so, eps2, 0.1, 2.0**-30, 2.0**-4, crit_order=crit)
         torch.cuda.synchronize()
         assert (tn_h, na_h) == (tn_g, na_g)
@@ -45,5 +46,5 @@ def test_step_host_equals_device_path_and_oracle(order):
             assert np.array_equal(h["D"][k], g.D[k].cpu().numpy())
         if blk == 0:  # identical inputs on the first block: same membership as the oracle, state within tolerance
             assert tn_h == tn_o and na_h == idx_o.shape[0]
-            assert np.max(np.abs(h["x"] - so.x)) < 1e-10 and np.max(np.abs(h["v"] - so.v)) < 1e-8
+            U.check_corrected(order, idx_o, h_old[idx_o], h["x"], h["v"], so.x, so.v, so.D)
     ctx.close()

@@ -183,3 +183,34 @@ def test_total_energy_helper_matches_definition():
             w -= c["m"][i] * c["m"][j] / math.sqrt(np.sum((c["x"][i] - c["x"][j]) ** 2) + c["eps2"])
     k = 0.5 * np.sum(c["m"] * np.sum(c["v"] ** 2, axis=1))
     assert e == pytest.approx(k + w, rel=1e-13)
+
+
+def test_force_abs_conditioning_numbers():
+    """c-16 diagnostic: kappa = Sum|term| / |Sum term| is exactly 1 for N = 2 (one term), >= 1 always (triangle
+    inequality), and large for a particle in the middle of a symmetric pair (near-total cancellation)."""
+    rng = np.random.default_rng(2)
+    m = np.array([0.5, 0.5])
+    x = np.array([[1.0, 0.2, 0.0], [-0.3, 0.0, 0.1]])
+    v = rng.normal(size=(2, 3))
+    a = rng.normal(size=(2, 3))
+    j = rng.normal(size=(2, 3))
+    idx = np.arange(2, dtype=np.int32)
+    f = O.force(m, x, v, a, j, idx, 8, 0.01)
+    ab = O.force_abs(m, x, v, a, j, idx, 8, 0.01)
+    for k in range(4):
+        np.testing.assert_allclose(ab[k], np.linalg.norm(f[k], axis=1), rtol=1e-14)
+    n = 40
+    m = rng.uniform(0.1, 1.0, n)
+    x, v, a, j = (rng.normal(size=(n, 3)) for _ in range(4))
+    idx = np.arange(n, dtype=np.int32)
+    f = O.force(m, x, v, a, j, idx, 8, 0.01)
+    ab = O.force_abs(m, x, v, a, j, idx, 8, 0.01)
+    for k in range(4):
+        assert np.all(ab[k] >= np.linalg.norm(f[k], axis=1) * (1 - 1e-14))
+    # a test particle midway between two equal masses at rest: acc cancels, kappa_acc is huge
+    m = np.array([1e-12, 1.0, 1.0])
+    x = np.array([[0.0, 0.0, 1e-9], [1.0, 0.0, 0.0], [-1.0, 0.0, 0.0]])
+    z = np.zeros((3, 3))
+    f = O.force(m, x, z, None, None, np.array([0], dtype=np.int32), 4, 0.0)
+    ab = O.force_abs(m, x, z, None, None, np.array([0], dtype=np.int32), 4, 0.0)
+    assert ab[0][0] / np.linalg.norm(f[0][0]) > 1e8 and abs(ab[0][0] - 2.0) < 1e-9

@@ -23,7 +23,10 @@ def test_shard_bounds_partition():
             assert cover[0][0] == 0 and cover[-1][1] == n_act
             assert all(cover[i][1] == cover[i + 1][0] for i in range(world - 1))
             sizes = [hi - lo for lo, hi in cover]
-            assert max(sizes) - min(sizes) <= 1
+            chunk = (n_act + world - 1) // world
+            # fixed chunks, the last non-empty one shorter: the gathered buffer is the record array in list order
+            assert max(sizes) == chunk
+            assert all(lo == min(r * chunk, n_act) for r, (lo, hi) in enumerate(cover))
 
 
 def _free_port():
@@ -87,6 +90,9 @@ class _OracleCtx:
         self.O, self.m = O, m
         self.pred = None
 
+    def set_option(self, key, value):
+        assert key == "geometry_n_act"  # the oracle's summation order does not depend on the partition
+
     def next_block(self, n, t, dt, active):
         tn, idx = self.O.next_block(t.numpy(), dt.numpy())
         active[: idx.shape[0]] = torch.from_numpy(idx)
@@ -131,23 +137,28 @@ def _make_state(order, n):
     return s, so
 
 
-def _step_worker(rank, world, port, order, n, nblk, out_dir):
+def _step_worker(rank, world, port, order, n, nblk, out_dir, force_exchange):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     s, _ = _make_state(order, n)
+    sent = 0
     for _ in range(nblk):
-        P.sharded_block_step(s, rank, world)
+        sent += P.sharded_block_step(s, rank, world, force_exchange=force_exchange)[2]
+    assert sent > 0 or not force_exchange
     np.savez(os.path.join(out_dir, "s%d.npz" % rank), t=s.t.numpy(), dt=s.dt.numpy(), x=s.x.numpy(), v=s.v.numpy(),
              pot=s.pot.numpy(), **{"D%d" % k: s.D[k].numpy() for k in range(order)})
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,order", [(2, 6), (3, 4)])
-def test_sharded_block_step_matches_single_process(tmp_path, world, order):
+@pytest.mark.parametrize("world,order,force_exchange", [(2, 6, True), (3, 4, True), (2, 8, False)])
+def test_sharded_block_step_matches_single_process(tmp_path, world, order, force_exchange):
+    """force_exchange: every block is sharded and exchanged; otherwise blocks below REDUNDANT_BELOW are computed by
+    every rank with no collective and only larger blocks are sharded."""
     from oracle import integrate as OI
     n, nblk = 193, 12
-    mp.spawn(_step_worker, args=(world, _free_port(), order, n, nblk, str(tmp_path)), nprocs=world, join=True)
+    mp.spawn(_step_worker, args=(world, _free_port(), order, n, nblk, str(tmp_path), force_exchange), nprocs=world,
+             join=True)
     _, so = _make_state(order, n)
     for _ in range(nblk):
         OI.block_step(so, 1e-6, 0.1, 2.0**-30, 2.0**-4, crit_order=4 if order >= 6 else 0)
