@@ -112,12 +112,13 @@ def test_full_size_physically_consistent_derivatives(config, order):
     g.ctx.predict(n, H, order, g.t, g.m, g.x, g.v, g.D)
     out = _force(g.ctx, g.all_idx, n, order, eps2)
     geo = g.ctx.last_force_geometry()
-    assert geo["j_lanes"] == 1 and geo["j_splits"] == 1
+    assert geo["j_lanes"] == 1 and (geo["j_splits"] == 1 or config == 3)  # configs 4 and 5: the unsplit launch bench.py times
     ii = torch.from_numpy(s.astype(np.int64)).cuda()
     got = tuple(None if a is None else a[ii].cpu().numpy() for a in out)
     radius = np.linalg.norm(c["x"][s], axis=1)
     rep = U.conditioning_report(got, ref, absn, radius, order)
-    line = dict(test="full_size_physically_consistent", config=config, n=n, order=order, sample=int(s.shape[0]), report=rep)
+    line = dict(test="full_size_physically_consistent", config=config, n=n, order=order, sample=int(s.shape[0]),
+                geometry=geo, report=rep)
     print(json.dumps(line))
     os.makedirs("gpurun_out", exist_ok=True)
     with open(os.path.join("gpurun_out", "parity_fullsize_cfg%d.json" % config), "w") as f:
