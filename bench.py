@@ -29,6 +29,9 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 CONV_FLOPS = {4: 60, 6: 97, 8: 144}  # flops per interaction, community convention (R13)
+SASS_FLOPS = {4: 41, 6: 78, 8: 127}  # executed: 2 x FFMA + FMUL + FADD + 3 DADD per pair in the loop's SASS (R13)
+PACKED_OPS = {4: 24, 6: 46, 8: 76}   # FFMA2 + FMUL2 + FADD2 per (thread, j) = per two pairs
+OTHER_OPS = {4: 19.5, 6: 20.5, 8: 21.5}  # DADD, F2F, MUFU, LDS, loop overhead per (thread, j)
 SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
 FP32_PEAK_TFLOPS = 2 * FP32_LANES * SM_COUNT * SM_MAX_GHZ / 1e3  # 74.45, "alu" roofline denominator
 METRIC = "6th-order Hermite force interactions/s at N=1M (all active), whole block step"
@@ -229,19 +232,28 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (K_force), measured live over the timed steps ----
     f_avg = f_s / args.steps
-    achieved = CONV_FLOPS[order] * mine * n / f_avg / 1e12
-    traffic = None
-    tj = os.path.join(ROOT, "profiles", "r01_force_traffic.json")
-    if os.path.exists(tj):
+    pairs_per_s = mine * n / f_avg
+    achieved = CONV_FLOPS[order] * pairs_per_s / 1e12
+    counters = {}
+    cj = os.path.join(ROOT, "profiles", "r02_force_counters.json")  # ncu capture of this launch (profiles/r02_force6_1M.md)
+    if os.path.exists(cj):
         try:
-            traffic = json.load(open(tj)).get("dram_bytes_per_launch")
+            counters = json.load(open(cj))
         except Exception:
-            traffic = None
-    roofline = {"bound": "alu", "kernel": "k_force<%d,%d,%d,%d>" % (order, geom["i_per_thread"], geom["j_lanes"], 0),
+            counters = {}
+    traffic = counters.get("dram_bytes_per_launch") if order == 6 and n == 1048576 and world == 1 else None
+    sass = SASS_FLOPS[order]
+    roofline = {"bound": "alu", "kernel": "k_force<%d, %d, 0>" % (order, geom["j_lanes"]),
                 "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
                 "traffic": traffic, "flops_per_interaction": CONV_FLOPS[order],
+                "flops_convention": "%d flops per interaction is the community convention for order %d (DESIGN.md R13; "
+                                    "not in PAPER.md); the kernel EXECUTES %d (SASS count: FFMA x2 + FMUL + FADD + DADD)"
+                                    % (CONV_FLOPS[order], order, sass),
+                "flops_sass": sass, "achieved_executed": sass * pairs_per_s / 1e12,
+                "frac_executed": sass * pairs_per_s / 1e12 / FP32_PEAK_TFLOPS,
                 "peak_source": "nominal 2*128*148*1.965 GHz (DESIGN.md section 6); HBM/bf16 peaks do not bound this kernel",
-                "kernel_ms": 1e3 * f_avg, "kernel_share_of_step": f_s / dev_s}
+                "kernel_ms": 1e3 * f_avg, "kernel_share_of_step": f_s / dev_s,
+                "pairs_per_s": pairs_per_s}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32 pair math, f64 differences and accumulation",
@@ -333,7 +345,23 @@ def main():
         # instruction-class micro-probes (1e12 thread-ops/s, SM MHz inside the probe): context for the roofline
         names = {0: "ffma", 5: "ffma2_two_fresh_operands", 6: "ffma2_three_fresh_operands", 1: "dadd",
                  2: "f2f_f64_f32_roundtrip", 3: "mufu_rsq"}
+        names.update({7: "ffma2_plus_shf_pair", 8: "ffma2_plus_dadd_pair", 9: "ffma2_plus_lds128_pair"})
         line["probes_tera_ops"] = {nm: [round(v, 3) for v in g.ctx.probe_peak(k, 150)] for k, nm in names.items()}
+        pr, rl = line["probes_tera_ops"], line["roofline"]
+        rl["peak_measured"] = 2.0 * pr["ffma"][0]  # Tflop/s of the FFMA probe on this chip, this run
+        rl["frac_measured_peak"] = rl["achieved"] / rl["peak_measured"]
+        rl["frac_executed_measured"] = rl["achieved_executed"] / rl["peak_measured"]
+        # issue-port model: a packed op holds the sub-partition's issue port for 2 cycles (probes 7-9:
+        # an instruction of another pipe next to an FFMA2 is NOT hidden behind its second cycle), so one (warp, j) costs at
+        # least 2 x packed + other issue cycles for 64 pairs
+        cyc = 2 * PACKED_OPS[order] + OTHER_OPS[order]
+        bound = 64.0 / cyc * 4 * SM_COUNT * SM_MAX_GHZ * 1e9
+        rl["issue_port_model"] = {"cycles_per_warp_j": cyc, "bound_pairs_per_s": bound,
+                                  "frac": rl["pairs_per_s"] / bound,
+                                  "fma_pipe_floor_pairs_per_s": 64.0 / (2 * PACKED_OPS[order]) * 4 * SM_COUNT * SM_MAX_GHZ * 1e9,
+                                  "pair_cost_vs_ffma2": {k: round(pr["ffma2_two_fresh_operands"][0] / pr[k][0], 3)
+                                                         for k in ("ffma2_plus_shf_pair", "ffma2_plus_dadd_pair",
+                                                                   "ffma2_plus_lds128_pair") if pr[k][0] > 0}}
         if not args.no_e2e:
             line["e2e"] = e2e_leg(args, g, c, order, eps2, H)
         if not args.no_cpu_baseline and world == 1:

@@ -383,6 +383,8 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
     __shared__ long long s_base, s_all;
     const unsigned grid = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // a stopped run stays stopped (nothing after the stopping selection touches the state): replays are no-ops
+    if (A.run_mode && *(volatile int *)&A.ctl->stop) return;
     const long long chunk = (A.n + grid - 1) / grid;
     const long long c0 = (long long)blockIdx.x * chunk;
     const long long c1 = c0 + chunk < A.n ? c0 + chunk : A.n;
@@ -1085,7 +1087,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     }
 
     // batches of block steps between two looks at the control block
-    int batch = 4;
+    int batch = 8;
     int rc = NBODY_OK;
     for (;;) {
         for (int b = 0; b < batch && rc == NBODY_OK; ++b) {

@@ -33,7 +33,6 @@
 namespace nbody {
 namespace {
 
-constexpr int kUnroll = 4;  // j-particles per unrolled group of the pair loop
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -282,26 +281,27 @@ template <int ORDER, int JL, int DIFF, bool MASK>
 __device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const uint4 *tq, int j0, int jl,
                                              const Consts &C, f2 (&pa)[3 * (ORDER / 2) + 1], double *acc_mine) {
     constexpr int JPT = kTileJ / JL;                 // j-particles per thread and tile
-    constexpr int G0 = ORDER == 8 ? 2 : 1;           // heads issued before their tails
-    constexpr int G = G0 < JPT ? G0 : JPT;
-    constexpr int U = (kUnroll < JPT ? kUnroll : JPT) / G;
+    constexpr int CH = JPT < 64 ? JPT : 64;          // fp32 partials are flushed to fp64 every <= 64 j (R10)
+    constexpr int G0 = ORDER >= 6 ? 2 : 1;           // heads issued before their tails (measured: +2 % at orders 6, 8)
+    constexpr int G = G0 < CH ? G0 : CH;
+    constexpr int kUnroll = ORDER >= 6 ? 8 : 4;      // j-particles per unrolled group (measured per order)
 #pragma unroll 1
-    for (int ub = 0; ub < JPT; ub += U * G) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
+    for (int jj0 = 0; jj0 < JPT; jj0 += CH) {
+#pragma unroll(kUnroll / G)
+        for (int u = 0; u < CH; u += G) {
             Stage S[G];
 #pragma unroll
             for (int g = 0; g < G; ++g) {
-                const int jt = (ub + u * G + g) * JL + jl;
+                const int jt = (jj0 + u + g) * JL + jl;
                 head<ORDER, DIFF, MASK>(I, tq, jt, j0 + jt, C, S[g]);
             }
 #pragma unroll
             for (int g = 0; g < G; ++g) {
-                const int jt = (ub + u * G + g) * JL + jl;
+                const int jt = (jj0 + u + g) * JL + jl;
                 tail<ORDER, DIFF>(I, tq, jt, C, S[g], pa);
             }
         }
-        if (JPT >= 64 && ((ub + U * G) % 64) == 0) flush(pa, acc_mine);
+        if (JPT >= 64) flush(pa, acc_mine);
     }
 }
 
@@ -319,7 +319,7 @@ __device__ __forceinline__ void force_item(const ForceArgs &A, const int n_act, 
     double *acc_sm = reinterpret_cast<double *>(smem_raw + G::TILE_BYTES);
     const uint32_t bar0 = smem_u32(smem_raw + G::TILE_BYTES + G::ACC_BYTES);
     const int tid = threadIdx.x;
-    const int il = tid % IT, jl = tid / IT;
+    const int il = JL == 1 ? tid : tid % IT, jl = JL == 1 ? 0 : tid / IT;  // JL = 1: uniform tile addresses (LDS [UR + imm])
     const int tile_lo = (int)((long long)A.n_tiles * split / splits);
     const int tile_hi = (int)((long long)A.n_tiles * (split + 1) / splits);
     const int ntile = tile_hi - tile_lo;
@@ -431,7 +431,7 @@ __device__ __forceinline__ void force_item(const ForceArgs &A, const int n_act, 
         const int comp = o / (2 * IT), rem = o % (2 * IT);
         const int r = rem / IT, i_l = rem % IT;
         double sum = 0.0;
-#pragma unroll 1
+#pragma unroll 8
         for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
         const int slot = i_tile * (2 * IT) + r * IT + i_l;
         if (slot < n_act) {
@@ -495,34 +495,57 @@ __global__ void __launch_bounds__(kThreads, 1) k_force_dyn(const ForceArgs A) {
     }
 }
 
-// K_reduce (a-3b): out = Sum_{s = 0 .. S-1} partial[s] in that order.
+// K_reduce (a-3b): out = Sum over the S j-splits of partial[s], in a FIXED order that depends on S only (so the result is
+// bit-reproducible and the same for every caller that uses the same S):
+//   S <= 8 : one thread per output, s = 0 .. S-1 in sequence;
+//   S  > 8 : one warp per output, lane l sums s = l, l + 32, ... in sequence, then a fixed butterfly over the lanes.
+__device__ __forceinline__ void reduce_store(double s, long long o, int nc, int n_act, double *acc, double *jerk,
+                                             double *snap, double *crk, double *pot) {
+    const int comp = (int)(o / n_act), slot = (int)(o % n_act);
+    if (comp == nc - 1) pot[slot] = s;
+    else {
+        double *dst = comp < 3 ? acc : comp < 6 ? jerk : comp < 9 ? snap : crk;
+        dst[(size_t)slot * 3 + comp % 3] = s;
+    }
+}
+
 __device__ __forceinline__ void reduce_body(const double *partials, int splits, int nc, int n_act, double *acc,
-                                            double *jerk, double *snap, double *crk, double *pot, long long o0,
-                                            long long stride) {
+                                            double *jerk, double *snap, double *crk, double *pot) {
     const long long tot = (long long)nc * n_act;
-    for (long long o = o0; o < tot; o += stride) {
-        double s = 0.0;
-        for (int k = 0; k < splits; ++k) s += partials[(size_t)k * tot + o];
-        const int comp = (int)(o / n_act), slot = (int)(o % n_act);
-        if (comp == nc - 1) pot[slot] = s;
-        else {
-            double *dst = comp < 3 ? acc : comp < 6 ? jerk : comp < 9 ? snap : crk;
-            dst[(size_t)slot * 3 + comp % 3] = s;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nthr = (long long)gridDim.x * blockDim.x;
+    if (splits <= 8) {
+        for (long long o = tid; o < tot; o += nthr) {
+            double v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = k < splits ? partials[(size_t)k * tot + o] : 0.0;
+            double s = v[0];
+#pragma unroll
+            for (int k = 1; k < 8; ++k)
+                if (k < splits) s += v[k];
+            reduce_store(s, o, nc, n_act, acc, jerk, snap, crk, pot);
+        }
+    } else {
+        const int lane = threadIdx.x & 31;
+        for (long long o = tid >> 5; o < tot; o += nthr >> 5) {
+            double s = 0.0;
+#pragma unroll 4
+            for (int k = lane; k < splits; k += 32) s += partials[(size_t)k * tot + o];
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+            if (lane == 0) reduce_store(s, o, nc, n_act, acc, jerk, snap, crk, pot);
         }
     }
 }
 
 __global__ void __launch_bounds__(256) k_reduce(const double *partials, int splits, int nc, int n_act, double *acc,
                                                 double *jerk, double *snap, double *crk, double *pot) {
-    reduce_body(partials, splits, nc, n_act, acc, jerk, snap, crk, pot,
-                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+    reduce_body(partials, splits, nc, n_act, acc, jerk, snap, crk, pot);
 }
 
 __global__ void __launch_bounds__(256) k_reduce_dyn(const Ctl *ctl, const double *partials, int nc, double *acc,
                                                     double *jerk, double *snap, double *crk, double *pot) {
     if (ctl->stop || ctl->splits == 1) return;
-    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot,
-                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot);
 }
 
 typedef void (*force_fn)(const ForceArgs);
@@ -613,7 +636,7 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
     NB_CUDA(c, cudaGetLastError());
     if (g.splits > 1) {
         const long long tot = (long long)NC * n_act;
-        long long blocks = (tot + 255) / 256;
+        long long blocks = g.splits <= 8 ? (tot + 255) / 256 : (tot + 7) / 8;  // thread or warp per output
         if (blocks > 8LL * c->sm_count) blocks = 8LL * c->sm_count;
         k_reduce<<<(unsigned)blocks, 256, 0, st>>>(c->partials, g.splits, NC, (int)n_act, acc, jerk, snap, crackle, pot);
         c->launches += 1;
@@ -633,7 +656,7 @@ int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, d
     fill_args(c, A, active_idx, eps2, acc, jerk, snap, crackle, pot);
     pick_dyn(order)<<<c->sm_count, kThreads, smem_for(order, 0), st>>>(A);
     NB_CUDA(c, cudaGetLastError());
-    k_reduce_dyn<<<2 * c->sm_count, 256, 0, st>>>(c->d_ctl, c->partials, NC, acc, jerk, snap, crackle, pot);
+    k_reduce_dyn<<<4 * c->sm_count, 256, 0, st>>>(c->d_ctl, c->partials, NC, acc, jerk, snap, crackle, pot);
     NB_CUDA(c, cudaGetLastError());
     return NBODY_OK;
 }

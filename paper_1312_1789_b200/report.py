@@ -3,9 +3,12 @@
     python -m paper_1312_1789_b200.report sweep --config {2,3,4} [--n N]
         force throughput per N_act (config 2: 1..65536 x16; config 3: 4^0..4^9; config 4: all-active + the
         log-uniform block-size histogram 2^0..2^20), one JSON line per call class
-    python -m paper_1312_1789_b200.report integrate --config 5 [--n N] [--t-end 0.0625] [--order P]
+    python -m paper_1312_1789_b200.report integrate --config 5 [--n N] [--t-end 0.0625] [--order P] [--driver host|device]
         end-to-end block-time-step integration (bootstrap, then select/predict/force/correct per block) with the
-        relative energy error, block-size histogram, time split and sustained Tflop/s
+        relative energy error, block-size histogram, time split (host driver) and sustained Tflop/s; --driver device
+        runs the blocks through nbody_run_blocks (CUDA graph per block step, no host round trip per block)
+    python -m paper_1312_1789_b200.report latency [--config 2] [--n 65536] [--order 4] [--blocks 400]
+        microseconds per block step over the same run of blocks: host-driven path against the device-driven path
 
 Product code only (no oracle): every step runs through the C ABI.  Inputs are the seeded synthetic clusters of
 workloads.py.
@@ -66,11 +69,28 @@ def sweep(args):
                       "algorithmic_GBps": bytes_pp * n / (med * 1e-3) / 1e9}), flush=True)
     out = [torch.zeros(n, 3, dtype=torch.float64, device="cuda") for _ in range(4)]
     pot = torch.zeros(n, dtype=torch.float64, device="cuda")
+    # the other O(N) kernels of a block step on an all-active block: selection (a-1) and corrector (a-4)
+    act = torch.zeros(n, dtype=torch.int32, device="cuda")
+    d_dt = _dev(dt)
+    med, best, _ = _time_call(lambda: ctx.next_block(n, st[0], d_dt, act))
+    print(json.dumps({"call": "next_block", "config": args.config, "n": n, "us": med * 1e3, "us_best": best * 1e3,
+                      "note": "one kernel + 168-byte D2H + stream synchronise", "algorithmic_GBps": 20 * n / (med * 1e-3) / 1e9}),
+          flush=True)
+    full = [_dev(d) for d in (D + [np.zeros_like(D[0])] * 8)[:8]]
+    sx, sv, sp, s_t, s_dt = st[2].clone(), st[3].clone(), torch.zeros(n, dtype=torch.float64, device="cuda"), st[0].clone(), d_dt.clone()
+    corr = lambda: ctx.correct(act, n, order, t_now, 0.1, 2.0**-30, 2.0**-4, s_t, s_dt, sx, sv, full, sp, dD[0], dD[1],
+                               dD[2] if order >= 6 else None, dD[3] if order >= 8 else None, pot)
+    med, best, _ = _time_call(corr)
+    bytes_pc = {4: 332, 6: 428, 8: 524}[order]
+    print(json.dumps({"call": "correct", "config": args.config, "n": n, "order": order, "n_act": n, "us": med * 1e3,
+                      "us_best": best * 1e3, "algorithmic_GBps": bytes_pc * n / (med * 1e-3) / 1e9}), flush=True)
     rng = W.rng_for(args.config, 41)
     if args.config == 2:
         nacts = [1, 16, 256, 4096, 65536]
     elif args.config == 3:
         nacts = [4**k for k in range(10)]
+    elif args.config == 5:
+        nacts = [1, 16, 256, 4096, 65536, n]
     else:
         nacts = [n]
     for n_act in nacts:
@@ -126,27 +146,37 @@ def integrate(args):
     marks, hist = [], {}
     w0 = time.perf_counter()
     pairs = 0
-    while True:
-        t_next, n_act = g.ctx.next_block(n, g.t, g.dt, g.active)
-        if t_next > args.t_end or (time.perf_counter() - w0) > args.max_seconds:
-            break
-        p = order
-        a, b, cc, d = ev(), ev(), ev(), ev()
-        a.record()
-        g.ctx.predict(n, t_next, p, g.t, g.m, g.x, g.v, g.D)
-        b.record()
-        g.ctx.force(g.active, n_act, p, eps2, g.acc, g.jerk, g.snap if p >= 6 else None, g.crk if p >= 8 else None,
-                    g.fpot)
-        cc.record()
-        g.ctx.correct(g.active, n_act, p, t_next, g.eta, g.dt_min, g.dt_max, g.t, g.dt, g.x, g.v, g.D, g.pot, g.acc,
-                      g.jerk, g.snap if p >= 6 else None, g.crk if p >= 8 else None, g.fpot)
-        d.record()
-        marks.append((a, b, cc, d))
-        g.time = t_next
-        g.blocks += 1
-        pairs += n_act * n
-        k = int(n_act).bit_length() - 1
-        hist[k] = hist.get(k, 0) + 1
+    if args.driver == "device":
+        while True:
+            r = g.run(args.t_end, max_blocks=1 << 16)
+            pairs += r["pairs"]
+            for k, v in enumerate(r["hist_log2"]):
+                if v:
+                    hist[k] = hist.get(k, 0) + v
+            if r["stop_reason"] != 3 or (time.perf_counter() - w0) > args.max_seconds:
+                break
+    else:
+        while True:
+            t_next, n_act = g.ctx.next_block(n, g.t, g.dt, g.active)
+            if t_next > args.t_end or (time.perf_counter() - w0) > args.max_seconds:
+                break
+            p = order
+            a, b, cc, d = ev(), ev(), ev(), ev()
+            a.record()
+            g.ctx.predict(n, t_next, p, g.t, g.m, g.x, g.v, g.D)
+            b.record()
+            g.ctx.force(g.active, n_act, p, eps2, g.acc, g.jerk, g.snap if p >= 6 else None, g.crk if p >= 8 else None,
+                        g.fpot)
+            cc.record()
+            g.ctx.correct(g.active, n_act, p, t_next, g.eta, g.dt_min, g.dt_max, g.t, g.dt, g.x, g.v, g.D, g.pot, g.acc,
+                          g.jerk, g.snap if p >= 6 else None, g.crk if p >= 8 else None, g.fpot)
+            d.record()
+            marks.append((a, b, cc, d))
+            g.time = t_next
+            g.blocks += 1
+            pairs += n_act * n
+            k = int(n_act).bit_length() - 1
+            hist[k] = hist.get(k, 0) + 1
     torch.cuda.synchronize()
     wall = time.perf_counter() - w0
     t_pred = sum(a.elapsed_time(b) for a, b, _, _ in marks) * 1e-3
@@ -155,25 +185,110 @@ def integrate(args):
     done = bool((g.t == args.t_end).all())
     e1 = g.energy() if bool((g.t == g.t[0]).all()) else float("nan")
     dts = g.dt.cpu().numpy()
-    print(json.dumps({"call": "integrate", "config": args.config, "n": n, "order": order, "eta": args.eta,
+    print(json.dumps({"call": "integrate", "driver": args.driver, "config": args.config, "n": n, "order": order, "eta": args.eta,
                       "dt_criterion_order": g.dt_criterion_order, "dt_max_log2": -args.dt_max_log2, "t_end": args.t_end, "reached_t_end": done,
                       "time_reached": g.time, "blocks": g.blocks, "pairs": pairs, "wall_s": wall,
-                      "bootstrap_s": t_boot, "split_s": {"predict": t_pred, "force": t_force, "correct": t_corr,
-                                                         "host_and_selection": wall - t_pred - t_force - t_corr},
+                      "bootstrap_s": t_boot,
+                      "split_s": ({"predict": t_pred, "force": t_force, "correct": t_corr,
+                                   "host_and_selection": wall - t_pred - t_force - t_corr} if marks else None),
                       "sustained_tflops_conventional": pairs * CONV_FLOPS[order] / wall / 1e12,
                       "sustained_frac_fp32_peak": pairs * CONV_FLOPS[order] / wall / FP32_PEAK,
-                      "force_only_tflops": pairs * CONV_FLOPS[order] / max(t_force, 1e-9) / 1e12,
+                      "force_only_tflops": (pairs * CONV_FLOPS[order] / max(t_force, 1e-9) / 1e12) if marks else None,
                       "E0": e0, "E1": e1, "rel_energy_error": abs((e1 - e0) / e0),
                       "block_size_histogram_log2": {str(k): v for k, v in sorted(hist.items())},
                       "dt_log2_min_median_max": [float(np.log2(dts.min())), float(np.log2(np.median(dts))),
                                                  float(np.log2(dts.max()))]}), flush=True)
 
 
+def latency(args):
+    """us per SMALL block step (n_act <= --small): the host-driven path (one selection round trip and 4-5 launches per
+    block) against the device-driven path (nbody_run_blocks), over the same sequence of blocks.  Larger blocks in
+    between are stepped untimed.  Wall-clock around synchronised calls."""
+    import torch
+    from . import workloads as W
+    from .scheduler import Integrator
+    c = W.cluster(args.config, args.n)
+    order = args.order or c["order"]
+    mk = lambda: Integrator(c["m"], c["x"], c["v"], order, c["eps2"], dt_max=2.0**-args.dt_max_log2)
+    res = {}
+    if args.synthetic:
+        # A run of small blocks only: `synthetic` particles nearest the centre restart on steps of 2^-16 while everybody
+        # else waits on 2^-4, so every block until t = 2^-4 is a subset of those particles (their steps grow back to the
+        # criterion's value on the way).  One call per driver over exactly the same blocks.
+        r0 = np.argsort(np.linalg.norm(c["x"], axis=1))[: args.synthetic]
+        for driver in ("host", "device", "device_nograph"):
+            g = mk()
+            g.bootstrap()
+            g.dt.fill_(2.0**-4)
+            g.dt[torch.from_numpy(r0).cuda()] = 2.0**-16
+            if driver == "device_nograph":
+                g.ctx.set_option("use_graph", 0)
+            t_stop = 2.0**-4 - 2.0**-17
+            g.run(t_stop, max_blocks=args.skip)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            if driver == "host":
+                b0 = g.blocks
+                g.integrate(t_stop, max_blocks=g.blocks + args.blocks)
+                torch.cuda.synchronize()
+                nb = g.blocks - b0
+            else:
+                nb = g.run(t_stop, max_blocks=args.blocks)["blocks"]
+                torch.cuda.synchronize()
+            dt_ = time.perf_counter() - t0
+            res[driver] = dict(us_per_block=1e6 * dt_ / max(1, nb), blocks=nb)
+            g.ctx.close()
+        print(json.dumps({"call": "latency_small_blocks_only", "config": args.config, "n": c["n"], "order": order,
+                          "n_act_max": args.synthetic, **res}), flush=True)
+        return
+    for driver in ("host", "device", "device_nograph"):
+        g = mk()
+        g.bootstrap()
+        if driver == "device_nograph":
+            g.ctx.set_option("use_graph", 0)
+        g.run(1e9, max_blocks=args.skip)  # leave the synchronised start-up blocks behind
+        torch.cuda.synchronize()
+        small, t_small, big, sizes = 0, 0.0, 0, []
+        while small < args.blocks:
+            if driver == "host":
+                t0 = time.perf_counter()
+                t_next, n_act = g.ctx.next_block(g.n, g.t, g.dt, g.active)
+                p = order
+                g.ctx.predict(g.n, t_next, p, g.t, g.m, g.x, g.v, g.D)
+                g.ctx.force(g.active, n_act, p, g.eps2, g.acc, g.jerk, g.snap if p >= 6 else None,
+                            g.crk if p >= 8 else None, g.fpot)
+                g.ctx.correct(g.active, n_act, p, t_next, g.eta, g.dt_min, g.dt_max, g.t, g.dt, g.x, g.v, g.D, g.pot,
+                              g.acc, g.jerk, g.snap if p >= 6 else None, g.crk if p >= 8 else None, g.fpot)
+                torch.cuda.synchronize()
+                dt_ = time.perf_counter() - t0
+                if n_act <= args.small:
+                    small += 1
+                    t_small += dt_
+                    sizes.append(n_act)
+                else:
+                    big += 1
+            else:
+                t0 = time.perf_counter()
+                r = g.run(1e9, max_blocks=args.blocks - small, max_n_act=args.small)
+                torch.cuda.synchronize()
+                t_small += time.perf_counter() - t0
+                small += r["blocks"]
+                if r["stop_reason"] == 2:
+                    g.block_step()
+                    big += 1
+        res[driver] = dict(us_per_small_block=1e6 * t_small / max(1, small), small_blocks=small, larger_blocks_between=big)
+        if sizes:
+            res[driver]["median_n_act"] = float(np.median(sizes))
+        g.ctx.close()
+    print(json.dumps({"call": "latency", "config": args.config, "n": c["n"], "order": order, "small": args.small,
+                      "skipped": args.skip, **res}), flush=True)
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(prog="paper_1312_1789_b200.report")
     sub = ap.add_subparsers(dest="cmd", required=True)
     s = sub.add_parser("sweep")
-    s.add_argument("--config", type=int, required=True, choices=[2, 3, 4])
+    s.add_argument("--config", type=int, required=True, choices=[2, 3, 4, 5])
     s.add_argument("--n", type=int, default=None)
     s.add_argument("--order", type=int, default=None)
     i = sub.add_parser("integrate")
@@ -185,8 +300,18 @@ def main(argv=None):
     i.add_argument("--dt-min-log2", type=int, default=30)
     i.add_argument("--dt-max-log2", type=int, default=4, help="dt_max = 2^-k (must divide t_end)")
     i.add_argument("--max-seconds", type=float, default=1500.0)
+    i.add_argument("--driver", default="host", choices=["host", "device"])
+    l = sub.add_parser("latency")
+    l.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    l.add_argument("--n", type=int, default=65536)
+    l.add_argument("--order", type=int, default=None)
+    l.add_argument("--blocks", type=int, default=400)
+    l.add_argument("--skip", type=int, default=50)
+    l.add_argument("--small", type=int, default=16, help="blocks up to this size are timed")
+    l.add_argument("--synthetic", type=int, default=0, help="K > 0: a run in which every block has <= K particles")
+    l.add_argument("--dt-max-log2", type=int, default=4)
     args = ap.parse_args(argv)
-    (sweep if args.cmd == "sweep" else integrate)(args)
+    {"sweep": sweep, "integrate": integrate, "latency": latency}[args.cmd](args)
 
 
 if __name__ == "__main__":
