@@ -85,6 +85,15 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 ascending (hence unique) and in [0, n), nbody_correct additionally that t[i] + dt[i] == t_now for
  *                 every active i; a violation returns NBODY_EINVAL before any arithmetic.  Synchronises `stream`.
  *   "use_graph"   1 = nbody_run_blocks replays its five launches as one CUDA graph [default]; 0 = plain launches
+ *   "step_reject_ratio" R14, a-posteriori step rejection (a reading added by this build; the paper is silent):
+ *                 0 = off [default], the textbook scheme.  R = 2^r in [2, 2^20]: if the criterion evaluated at the END of
+ *                 a particle's step asks for dt_new <= h/R and h/R >= dt_min, nbody_correct does not take the step: x, v,
+ *                 a_derivs, pot_state and t of that particle keep their values and only dt := h/R is written.  The
+ *                 particle is then due at t + h/R, BEFORE the current block time: nbody_next_block / nbody_run_blocks pick
+ *                 it next and nbody_predict extrapolates everybody else back to that time (tau < 0 is legal).  Guards the
+ *                 end-point quadrature against encounters the start-of-step criterion could not see (a perturber at its
+ *                 closest approach on the end point of a long step: end-point derivatives m v^k / r^(k+2) times h^(k+1)).
+ *                 Bit-exact against the oracle's reject_ratio.  Count: nbody_rejected_steps / nbody_run_result.rejected.
  */
 int nbody_set_option(nbody_ctx *ctx, const char *key, int64_t value);
 
@@ -174,6 +183,10 @@ int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double 
 int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
                      int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);
 
+/* Steps refused by the "step_reject_ratio" rule since the counter was last reset (nbody_run_blocks resets it at the
+ * start of every run); reset != 0 clears it.  *count_host is a HOST pointer; synchronises `stream`. */
+int nbody_rejected_steps(nbody_ctx *ctx, int reset, int64_t *count_host, void *stream);
+
 /* Test hook: export the packed j-store of the last predict (n particles) into plain arrays.  xp fp64 [n][3];
  * vp, ap, jp fp32 [n][3] (ap/jp may be NULL; ap requires order >= 6, jp order == 8 else EINVAL); m32 fp32 [n]. */
 int nbody_get_predicted(nbody_ctx *ctx, double *xp, float *vp, float *ap, float *jp, float *m32, void *stream);
@@ -231,6 +244,7 @@ typedef struct nbody_run_result {
     int64_t n_act_next;
     int32_t stop_reason;
     int32_t reserved;
+    int64_t rejected;       /* steps refused by the "step_reject_ratio" rule during this run */
     int64_t hist_log2[40];
 } nbody_run_result;
 

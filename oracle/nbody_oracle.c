@@ -350,6 +350,15 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
  * call computes directly enter the step decision.  Added after the CUDA path showed that with fp32 pair arithmetic (c-12) the interpolated
  * a^(K..2K-1) of p >= 6 are rounding-noise dominated at small h and the order-p criterion collapses dt.
  *
+ * c-9b (R14, a reading added in round 2; the paper is silent, PAPER.md:15 says only "individual
+ * hierarchically block time-steps"): a-posteriori step rejection.  reject_ratio R = 0 switches it off (the textbook
+ * scheme); R = 2^r >= 2: if the criterion evaluated at the END of the step asks for dt_new <= h/R (the step was at
+ * least R times longer than the scheme now thinks it should have been: an encounter the start-of-step criterion
+ * could not see) and h/R >= dt_min, the step is NOT taken: x, v, D, pot_state and t of the particle keep their
+ * values at t0 and only dt := h/R is written.  The particle is then due at t0 + h/R, which lies BEFORE the current
+ * block time: the scheduler (c-11, min over t + dt) picks it next and the other particles are predicted back to
+ * that time with their own polynomials.  *n_rejected (may be NULL) is incremented per rejection.
+ *
  * State arrays (in/out, [n][3] unless noted): t[n], dt[n], x, v, D[k] = a^(k)
  * for k = 0..p-1, pot_state[n].  Force arrays in active-list order [n_act][3].
  * ------------------------------------------------------------------------ */
@@ -358,7 +367,8 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                     double *t, double *dt, double *x, double *v, double *const *D,
                     double *pot_state,
                     const double *acc, const double *jerk, const double *snap,
-                    const double *crackle, const double *pot, int variant, int crit_order)
+                    const double *crackle, const double *pot, int variant, int crit_order,
+                    int reject_ratio, int64_t *n_rejected)
 {
     const int p = order;
     /* c-8b (R8b): the criterion may be evaluated on the lowest pc <= p derivatives only.
@@ -367,12 +377,13 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
     const int pc = (crit_order == 4 || crit_order == 6 || crit_order == 8)
                        ? (crit_order < p ? crit_order : p)
                        : (p >= 6 ? 4 : p);
-#pragma omp parallel for schedule(static)
+    int64_t rejected = 0;
+#pragma omp parallel for schedule(static) reduction(+ : rejected)
     for (int64_t ia = 0; ia < n_act; ++ia) {
         const int64_t i = active_idx[ia];
         const double h = dt[i];
         const double h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h, h6 = h5 * h, h7 = h6 * h;
-        double dnew[8][3];
+        double dnew[8][3], xnew[3], vnew[3];
         double cbar[3] = {0.0, 0.0, 0.0}; /* c-8b, p = 6: mean crackle over the step, (s1 - s0)/h */
         for (int c = 0; c < 3; ++c) {
             const int64_t q = 3 * i + c, qa = 3 * ia + c;
@@ -421,19 +432,29 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                 dnew[0][c] = a1; dnew[1][c] = j1; dnew[2][c] = s1; dnew[3][c] = c1;
                 dnew[4][c] = A4; dnew[5][c] = A5; dnew[6][c] = A6; dnew[7][c] = A7;
             }
-            x[q] = x1;
-            v[q] = v1;
+            xnew[c] = x1;
+            vnew[c] = v1;
         }
         const double *dp[8];
         for (int k = 0; k < p; ++k) dp[k] = dnew[k];
         if (p == 6 && pc == 4) dp[3] = cbar; /* only directly computed derivatives enter the criterion */
         const double dt_new = oracle_new_dt(pc, dp, t_now, h, eta, dt_min, dt_max);
+        if (reject_ratio >= 2 && dt_new * (double)reject_ratio <= h && h / (double)reject_ratio >= dt_min) {
+            dt[i] = h / (double)reject_ratio; /* c-9b: the step is not taken; everything else stays at t0 */
+            rejected += 1;
+            continue;
+        }
+        for (int c = 0; c < 3; ++c) {
+            x[3 * i + c] = xnew[c];
+            v[3 * i + c] = vnew[c];
+        }
         for (int k = 0; k < p; ++k)
             for (int c = 0; c < 3; ++c) D[k][3 * i + c] = dnew[k][c];
         pot_state[i] = pot[ia];
         t[i] = t_now;
         dt[i] = dt_new;
     }
+    if (n_rejected) *n_rejected += rejected;
 }
 
 /* ------------------------------------------------------------------------ *

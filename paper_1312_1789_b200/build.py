@@ -19,7 +19,7 @@ UNITS = {
     "nbody_force.cu": ["-ftz=true"],
     "nbody_probe.cu": [],
 }
-HEADERS = [os.path.join(CSRC, "nbody_internal.h"), os.path.join(ROOT, "include", "nbody.h"),
+HEADERS = [os.path.join(CSRC, "nbody_internal.h"), os.path.join(CSRC, "nbody_exact.cuh"), os.path.join(ROOT, "include", "nbody.h"),
            os.path.join(ROOT, "include", "nbody_bench.h")]
 
 

@@ -11,20 +11,12 @@
 
 #include <new>
 
+#include "nbody_exact.cuh"
 #include "nbody_internal.h"
 
 using namespace nbody;
 
 namespace {
-
-__device__ __forceinline__ double dadd(double a, double b) { return __dadd_rn(a, b); }
-__device__ __forceinline__ double dsub(double a, double b) { return __dsub_rn(a, b); }
-__device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
-__device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
-__device__ __forceinline__ double dsqrt(double a) { return __dsqrt_rn(a); }
-
-// exact 2^e for e in the normal range [-1022, 1023] (the callers validate (|k| + 1) q <= 1022 on the host)
-__device__ __forceinline__ double pow2i(int e) { return __longlong_as_double((long long)(e + 1023) << 52); }
 
 struct PredArgs {
     const double *t, *m, *x, *v;
@@ -35,28 +27,6 @@ struct PredArgs {
     int write_ds;
     const Ctl *ctl;  // device-driven step: t_now = ctl->t_next, no-op when the run has stopped (else NULL)
 };
-
-__device__ __forceinline__ uint4 pack_dd(double a, double b) {
-    uint4 r;
-    long long ia = __double_as_longlong(a), ib = __double_as_longlong(b);
-    r.x = (unsigned)(ia & 0xffffffffll);
-    r.y = (unsigned)((unsigned long long)ia >> 32);
-    r.z = (unsigned)(ib & 0xffffffffll);
-    r.w = (unsigned)((unsigned long long)ib >> 32);
-    return r;
-}
-__device__ __forceinline__ uint4 pack_dff(double a, float b, float c) {
-    uint4 r;
-    long long ia = __double_as_longlong(a);
-    r.x = (unsigned)(ia & 0xffffffffll);
-    r.y = (unsigned)((unsigned long long)ia >> 32);
-    r.z = __float_as_uint(b);
-    r.w = __float_as_uint(c);
-    return r;
-}
-__device__ __forceinline__ uint4 pack_ffff(float a, float b, float c, float d) {
-    return make_uint4(__float_as_uint(a), __float_as_uint(b), __float_as_uint(c), __float_as_uint(d));
-}
 
 // K_pred: one thread per j-store slot (particles, then pads).  R5: Horner, innermost first, c_k = tau / k.
 template <int ORDER>
@@ -71,39 +41,10 @@ __global__ void __launch_bounds__(256) k_predict(PredArgs A) {
     double xp[3];
     float vp[3], ap[3] = {0.f, 0.f, 0.f}, jp[3] = {0.f, 0.f, 0.f}, m32 = 0.f;
     if (i < A.n) {
-        constexpr int ND = ORDER - 2;
-        const double tau = dsub(t_now, A.t[i]);
-        double c[9];
+        const double *Dp[6];
 #pragma unroll
-        for (int k = 1; k <= 8; ++k) c[k] = ddiv(tau, (double)k);
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            const long long q = 3 * i + d;
-            double Dk[ND];
-#pragma unroll
-            for (int k = 0; k < ND; ++k) Dk[k] = A.D[k][q];
-            double s = Dk[ND - 1];
-#pragma unroll
-            for (int k = ND - 1; k >= 1; --k) s = dadd(Dk[k - 1], dmul(c[k + 2], s));
-            const double vq = A.v[q];
-            xp[d] = dadd(A.x[q], dmul(tau, dadd(vq, dmul(c[2], s))));
-            s = Dk[ND - 1];
-#pragma unroll
-            for (int k = ND - 1; k >= 1; --k) s = dadd(Dk[k - 1], dmul(c[k + 1], s));
-            vp[d] = __double2float_rn(dadd(vq, dmul(tau, s)));
-            if (ORDER >= 6) {
-                s = Dk[ND - 1];
-#pragma unroll
-                for (int k = ND - 1; k >= 1; --k) s = dadd(Dk[k - 1], dmul(c[k], s));
-                ap[d] = __double2float_rn(s);
-            }
-            if (ORDER >= 8) {
-                s = Dk[ND - 1];
-#pragma unroll
-                for (int k = ND - 1; k >= 2; --k) s = dadd(Dk[k - 1], dmul(c[k - 1], s));
-                jp[d] = __double2float_rn(s);
-            }
-        }
+        for (int k = 0; k < ORDER - 2; ++k) Dp[k] = A.D[k] + 3 * i;
+        predict_particle<ORDER>(d_sub(t_now, A.t[i]), A.x + 3 * i, A.v + 3 * i, Dp, xp, vp, ap, jp);
         m32 = __double2float_rn(A.m[i]);
     } else {
         xp[0] = xp[1] = xp[2] = kPadPos;
@@ -118,7 +59,7 @@ __global__ void __launch_bounds__(256) k_predict(PredArgs A) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             hi[d] = __double2float_rn(xp[d]);
-            lo[d] = __double2float_rn(dsub(xp[d], (double)hi[d]));
+            lo[d] = __double2float_rn(d_sub(xp[d], (double)hi[d]));
         }
         A.q[4][i] = pack_ffff(hi[0], lo[0], hi[1], lo[1]);
         A.q[5][i] = pack_ffff(hi[2], lo[2], m32, vp[0]);
@@ -155,157 +96,8 @@ __global__ void k_unpack(const uint4 *q0, const uint4 *q1, const uint4 *q2, cons
 
 }  // namespace
 
-// ---------------------------------------------------------------------------------------------------------
-// K_corr (a-4): R6 corrector, R7 interpolated derivatives, R8 criterion, R9 quantisation.
-// ---------------------------------------------------------------------------------------------------------
+// K_pred's particle arithmetic and the whole of K_corr (k_correct, correct_one) live in nbody_exact.cuh.
 namespace {
-
-#define P_(a, b) dadd((a), (b))
-#define S_(a, b) dsub((a), (b))
-#define M_(a, b) dmul((a), (b))
-#define Q_(a, b) ddiv((a), (b))
-
-__device__ __forceinline__ double nrm3(const double *a) {
-    return dsqrt(P_(P_(M_(a[0], a[0]), M_(a[1], a[1])), M_(a[2], a[2])));
-}
-
-// R9 step 1: largest k in [k_lo, k_hi] with Ap * 2^(k q) <= A1 * E, else k_lo - 1 (NaN: every comparison false).
-__device__ __forceinline__ int floor_log2_ratio(double A1, double Ap, double E, int q, int k_lo, int k_hi) {
-    const double rhs = M_(A1, E);
-    int k = k_hi;
-    while (k >= k_lo && !(M_(Ap, pow2i(k * q)) <= rhs)) --k;
-    return k;
-}
-
-// R8 + R9 for one particle; d[k] = a^(k)(t1), k = 0..p-1
-template <int ORDER>
-__device__ __forceinline__ double new_dt(const double (*d)[3], double t1, double dt_old, double eta, int k_min,
-                                         int k_max, double dt_min, double dt_max) {
-    constexpr int p = ORDER, q = p - 3;
-    const double n0 = nrm3(d[0]), n1 = nrm3(d[1]), n2 = nrm3(d[2]);
-    const double m3 = nrm3(d[p - 3]), m2 = nrm3(d[p - 2]), m1 = nrm3(d[p - 1]);
-    const double A1 = dsqrt(P_(M_(n0, n2), M_(n1, n1)));
-    const double Ap = dsqrt(P_(M_(m3, m1), M_(m2, m2)));
-    double E = 1.0;
-#pragma unroll
-    for (int k = 0; k < q; ++k) E = M_(E, eta);
-    const int k = floor_log2_ratio(A1, Ap, E, q, k_min - 1, k_max + 1);
-    double dt_new = pow2i(k);
-    const double two_old = M_(2.0, dt_old);
-    if (dt_new > two_old) dt_new = two_old;
-    if (dt_new == two_old) {
-        const double r = Q_(t1, dt_new);  // exact: dt_new is a power of two
-        if (r != rint(r)) dt_new = dt_old;
-    }
-    if (dt_new > dt_max) dt_new = dt_max;
-    if (dt_new < dt_min) dt_new = dt_min;
-    return dt_new;
-}
-
-struct CorrArgs {
-    const int32_t *idx;
-    long long n_act;
-    double t_now, eta, dt_min, dt_max;
-    int k_min, k_max;
-    int crit_order;  // R8b: criterion evaluated on the lowest crit_order derivatives (<= ORDER)
-    double *t, *dt, *x, *v, *D[8], *pot_state;
-    const double *acc, *jerk, *snap, *crk, *pot;
-    const Ctl *ctl;  // device-driven step: n_act and t_now from the control block (else NULL)
-};
-
-template <int ORDER>
-__device__ __forceinline__ void correct_one(const CorrArgs &A, long long ia, double t_now);
-
-template <int ORDER>
-__global__ void __launch_bounds__(128) k_correct(CorrArgs A) {
-    long long n_act = A.n_act;
-    double t_now = A.t_now;
-    if (A.ctl) {
-        if (A.ctl->stop) return;
-        n_act = A.ctl->n_act;
-        t_now = A.ctl->t_next;
-    }
-    for (long long ia = (long long)blockIdx.x * blockDim.x + threadIdx.x; ia < n_act;
-         ia += (long long)gridDim.x * blockDim.x)
-        correct_one<ORDER>(A, ia, t_now);
-}
-
-template <int ORDER>
-__device__ __forceinline__ void correct_one(const CorrArgs &A, const long long ia, const double t_now) {
-    const long long i = A.idx[ia];
-    const double h = A.dt[i];
-    const double h2 = M_(h, h), h3 = M_(h2, h), h4 = M_(h3, h), h5 = M_(h4, h), h6 = M_(h5, h), h7 = M_(h6, h);
-    double dn[8][3];
-    double cbar[3] = {0.0, 0.0, 0.0};  // R8b, p = 6: mean crackle over the step, (s1 - s0) / h
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const long long q = 3 * i + c, qa = 3 * ia + c;
-        const double x0 = A.x[q], v0 = A.v[q];
-        const double a0 = A.D[0][q], j0 = A.D[1][q];
-        const double a1 = A.acc[qa], j1 = A.jerk[qa];
-        const double dl = S_(a0, a1);
-        const double hh = Q_(h, 2.0);
-        double v1, x1;
-        if (ORDER == 4) {
-            const double w = Q_(h2, 12.0);
-            v1 = P_(v0, P_(M_(hh, P_(a0, a1)), M_(w, S_(j0, j1))));
-            x1 = P_(x0, P_(M_(hh, P_(v0, v1)), M_(w, S_(a0, a1))));
-            const double A2 = Q_(M_(2.0, P_(P_(M_(3.0, dl), M_(h, j0)), M_(M_(2.0, h), j1))), h2);
-            const double A3 = Q_(M_(6.0, P_(P_(M_(2.0, dl), M_(h, j0)), M_(h, j1))), h3);
-            dn[0][c] = a1; dn[1][c] = j1; dn[2][c] = A2; dn[3][c] = A3;
-        } else if (ORDER == 6) {
-            const double s0 = A.D[2][q], s1 = A.snap[qa];
-            const double w2 = Q_(h2, 10.0), w3 = Q_(h3, 120.0);
-            v1 = P_(v0, P_(M_(hh, P_(a0, a1)), P_(M_(w2, S_(j0, j1)), M_(w3, P_(s0, s1)))));
-            x1 = P_(x0, P_(M_(hh, P_(v0, v1)), P_(M_(w2, S_(a0, a1)), M_(w3, P_(j0, j1)))));
-            const double A3 = Q_(M_(-3.0, S_(P_(P_(P_(M_(20.0, dl), M_(M_(8.0, h), j0)), M_(M_(12.0, h), j1)), M_(h2, s0)), M_(M_(3.0, h2), s1))), h3);
-            const double A4 = Q_(M_(-12.0, S_(P_(P_(P_(M_(30.0, dl), M_(M_(14.0, h), j0)), M_(M_(16.0, h), j1)), M_(M_(2.0, h2), s0)), M_(M_(3.0, h2), s1))), h4);
-            const double A5 = Q_(M_(-60.0, S_(P_(P_(P_(M_(12.0, dl), M_(M_(6.0, h), j0)), M_(M_(6.0, h), j1)), M_(h2, s0)), M_(h2, s1))), h5);
-            dn[0][c] = a1; dn[1][c] = j1; dn[2][c] = s1; dn[3][c] = A3; dn[4][c] = A4; dn[5][c] = A5;
-            cbar[c] = Q_(S_(s1, s0), h);
-        } else {
-            const double s0 = A.D[2][q], s1 = A.snap[qa];
-            const double c0 = A.D[3][q], c1 = A.crk[qa];
-            const double w2 = Q_(M_(3.0, h2), 28.0), w3 = Q_(h3, 84.0), w4 = Q_(h4, 1680.0);
-            v1 = P_(v0, P_(M_(hh, P_(a0, a1)), P_(M_(w2, S_(j0, j1)), P_(M_(w3, P_(s0, s1)), M_(w4, S_(c0, c1))))));
-            x1 = P_(x0, P_(M_(hh, P_(v0, v1)), P_(M_(w2, S_(a0, a1)), P_(M_(w3, P_(j0, j1)), M_(w4, S_(s0, s1))))));
-#define HERM8(k0, kj0, kj1, ks0, ks1, kc0, kc1)                                                                     \
-    P_(P_(S_(P_(P_(P_(M_(k0, dl), M_(M_(kj0, h), j0)), M_(M_(kj1, h), j1)), M_(M_(ks0, h2), s0)), M_(M_(ks1, h2), s1)), \
-          kc0),                                                                                                   \
-       kc1)
-            const double A4 = Q_(M_(4.0, HERM8(210.0, 90.0, 120.0, 15.0, 30.0, M_(h3, c0), M_(M_(4.0, h3), c1))), h4);
-            const double A5 = Q_(M_(60.0, HERM8(168.0, 78.0, 90.0, 14.0, 20.0, M_(h3, c0), M_(M_(2.0, h3), c1))), h5);
-            const double A6 = Q_(M_(120.0, HERM8(420.0, 204.0, 216.0, 39.0, 45.0, M_(M_(3.0, h3), c0), M_(M_(4.0, h3), c1))), h6);
-            const double A7 = Q_(M_(840.0, HERM8(120.0, 60.0, 60.0, 12.0, 12.0, M_(h3, c0), M_(h3, c1))), h7);
-#undef HERM8
-            dn[0][c] = a1; dn[1][c] = j1; dn[2][c] = s1; dn[3][c] = c1;
-            dn[4][c] = A4; dn[5][c] = A5; dn[6][c] = A6; dn[7][c] = A7;
-        }
-        A.x[q] = x1;
-        A.v[q] = v1;
-    }
-    double dt_new;
-    if (ORDER == 6 && A.crit_order == 4) {  // only directly computed derivatives enter the step decision
-        double d4[4][3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            d4[0][c] = dn[0][c]; d4[1][c] = dn[1][c]; d4[2][c] = dn[2][c]; d4[3][c] = cbar[c];
-        }
-        dt_new = new_dt<4>(d4, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
-    } else if (ORDER >= 8 && A.crit_order == 4)
-        dt_new = new_dt<4>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
-    else if (ORDER >= 8 && A.crit_order == 6)
-        dt_new = new_dt<6>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
-    else
-        dt_new = new_dt<ORDER>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
-#pragma unroll
-    for (int k = 0; k < ORDER; ++k)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) A.D[k][3 * i + c] = dn[k][c];
-    A.pot_state[i] = A.pot[ia];
-    A.t[i] = t_now;
-    A.dt[i] = dt_new;
-}
 
 // R9b start-up step
 __global__ void k_initial_dt(long long n, const double *acc, const double *jerk, double eta_s, int k_min, int k_max,
@@ -373,7 +165,8 @@ struct SelArgs {
     int n_tiles, sm_count, force_lanes, force_split;
     long long rows_budget;
     // run control
-    int run_mode;         // 0 = plain selection (never stops); 1 = run: honour t_end / max_blocks / max_n_act
+    int run_mode;         // 0 = plain selection (never stops); 1 = run: honour t_end / max_blocks / max_n_act;
+                          // 2 = as 1, and stop (4) in front of a block that does not fit one i-tile (fused run, N1)
     long long max_n_act;  // run: a block larger than this stops the run (stop = 2) for the host to handle
 };
 
@@ -480,6 +273,7 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
         else if ((long long)ctl->blocks >= ctl->max_blocks) stop = 3;
     }
     ForceGeo g = force_geometry(n_act, A.n_tiles, A.sm_count, A.force_lanes, /*force_split=*/1, A.rows_budget);
+    if (A.run_mode == 2 && !stop && g.i_tiles != 1) stop = 4;  // fused small-block run: this block needs the general step
     const long long slots = A.sm_count;
     long long S = 1;
     if (A.force_split) S = A.force_split;
@@ -656,6 +450,8 @@ int launch_correct(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, 
     for (int k = 0; k < 8; ++k) A.D[k] = k < order ? a_derivs[k] : nullptr;
     A.acc = acc; A.jerk = jerk; A.snap = snap; A.crk = crackle; A.pot = pot;
     A.ctl = ctl;
+    A.reject_ratio = c->reject_ratio;
+    A.n_rejected = &c->d_ctl->rejected;
     long long blocks = ctl ? 2LL * c->sm_count : (n_act + 127) / 128;
     if (blocks > 16LL * c->sm_count) blocks = 16LL * c->sm_count;
     if (order == 4) k_correct<4><<<(unsigned)blocks, 128, 0, st>>>(A);
@@ -767,6 +563,7 @@ int nbody_destroy(nbody_ctx *h) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph_small) cudaGraphExecDestroy(c->graph_small);
     if (h->ev_in) cudaEventDestroy(h->ev_in);
     if (h->ev_out) cudaEventDestroy(h->ev_out);
     if (h->run_stream) cudaStreamDestroy(h->run_stream);
@@ -826,6 +623,16 @@ int nbody_set_option(nbody_ctx *h, const char *key, int64_t value) {
     if (!strcmp(key, "validate")) {
         if (value != 0 && value != 1) return NBODY_EINVAL;
         c->validate = (int)value;
+        return NBODY_OK;
+    }
+    if (!strcmp(key, "step_reject_ratio")) {
+        if (value != 0 && (value < 2 || value > (1 << 20) || (value & (value - 1)) != 0)) return NBODY_EINVAL;
+        c->reject_ratio = (int)value;
+        return NBODY_OK;
+    }
+    if (!strcmp(key, "use_fused")) {
+        if (value != 0 && value != 1) return NBODY_EINVAL;
+        c->use_fused = (int)value;
         return NBODY_OK;
     }
     if (!strcmp(key, "use_graph")) {
@@ -956,6 +763,19 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
     return NBODY_OK;
 }
 
+int nbody_rejected_steps(nbody_ctx *h, int reset, int64_t *count_host, void *stream) {
+    if (!h || !count_host) return NBODY_EINVAL;
+    Ctx *c = &h->c;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long v = 0;
+    NB_CUDA(c, cudaMemcpyAsync(&v, &c->d_ctl->rejected, sizeof(v), cudaMemcpyDeviceToHost, st));
+    if (reset) NB_CUDA(c, cudaMemsetAsync(&c->d_ctl->rejected, 0, sizeof(v), st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    *count_host = (int64_t)v;
+    return NBODY_OK;
+}
+
 // ---- row records for the multi-GPU exchange -----------------------------------------------------------------
 static int rows_call(nbody_ctx *h, bool pack, const int32_t *idx, int64_t n_rows, int order, double *t, double *dt,
                      double *pot_state, double *x, double *v, double *const a_derivs[8], double *rec, void *stream) {
@@ -1036,10 +856,20 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     hc->max_blocks = max_blocks;
     NB_CUDA(c, cudaMemcpyAsync(c->d_ctl, hc, sizeof(Ctl), cudaMemcpyHostToDevice, st));
 
-    SelArgs SA;
+    SelArgs SA, SF;
     fill_select(h, SA, n, t, dt, active_idx, /*run_mode=*/1, max_n_act);
+    fill_select(h, SF, n, t, dt, active_idx, /*run_mode=*/2, max_n_act);
     const int sgrid = select_grid(c, n);
-    auto enqueue_step = [&](cudaStream_t s) -> int {
+    CorrArgs CA;  // the corrector's arguments in control-block mode (shared by K_corr and the fused step)
+    {
+        CA.idx = active_idx; CA.n_act = 0; CA.t_now = 0.0; CA.eta = eta; CA.dt_min = dt_min; CA.dt_max = dt_max;
+        CA.k_min = kmin; CA.k_max = kmax; CA.crit_order = criterion_order(c, order);
+        CA.t = t; CA.dt = dt; CA.x = x; CA.v = v; CA.pot_state = pot_state;
+        for (int k = 0; k < 8; ++k) CA.D[k] = k < order ? a_derivs[k] : nullptr;
+        CA.acc = acc; CA.jerk = jerk; CA.snap = snap; CA.crk = crackle; CA.pot = pot;
+        CA.ctl = c->d_ctl; CA.reject_ratio = c->reject_ratio; CA.n_rejected = &c->d_ctl->rejected;
+    }
+    auto enqueue_step = [&](cudaStream_t s) -> int {  // general step: any block size
         k_select<<<sgrid, kSelThreads, 0, s>>>(SA);
         NB_CUDA(c, cudaGetLastError());
         int rc = launch_predict(c, n, 0.0, order, t, m, x, v, a_derivs, c->d_ctl, s);
@@ -1049,9 +879,17 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         return launch_correct(c, active_idx, 0, order, 0.0, eta, dt_min, dt_max, kmin, kmax, t, dt, x, v, a_derivs,
                               pot_state, acc, jerk, snap, crackle, pot, c->d_ctl, s);
     };
-    constexpr int kStepLaunches = 5;  // k_select, k_predict, k_force_dyn, k_reduce_dyn, k_correct
+    auto enqueue_fused = [&](cudaStream_t s) -> int {  // N1: blocks that fit one i-tile, two launches
+        k_select<<<sgrid, kSelThreads, 0, s>>>(SF);
+        NB_CUDA(c, cudaGetLastError());
+        return launch_step_fused(c, order, (float)eps2, active_idx, t, m, x, v, a_derivs, CA, acc, jerk, snap, crackle,
+                                 pot, s);
+    };
+    constexpr int kStepLaunches = 5;   // k_select, k_predict, k_force_dyn, k_reduce_dyn, k_correct
+    constexpr int kFusedLaunches = 2;  // k_select, k_step_fused
+    const bool fused = c->use_fused != 0;
 
-    // one CUDA graph of the five launches, re-captured when any argument differs from the cached one
+    // CUDA graphs of the two step flavours, re-captured when any argument differs from the cached ones
     unsigned long long key[24] = {(unsigned long long)n, (unsigned long long)order, 0, 0, 0, 0,
                                   (unsigned long long)(uintptr_t)t, (unsigned long long)(uintptr_t)dt,
                                   (unsigned long long)(uintptr_t)m, (unsigned long long)(uintptr_t)x,
@@ -1060,49 +898,60 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
                                   (unsigned long long)(uintptr_t)jerk, (unsigned long long)(uintptr_t)snap,
                                   (unsigned long long)(uintptr_t)crackle, (unsigned long long)(uintptr_t)pot,
                                   (unsigned long long)max_n_act,
-                                  (unsigned long long)c->crit_order << 32 | (unsigned long long)c->force_lanes << 16 |
-                                      (unsigned long long)c->force_split,
+                                  (unsigned long long)c->reject_ratio << 40 | (unsigned long long)c->crit_order << 32 |
+                                      (unsigned long long)c->force_lanes << 16 | (unsigned long long)c->force_split,
                                   0, 0, 0, 0};
     memcpy(&key[2], &eps2, 8); memcpy(&key[3], &eta, 8); memcpy(&key[4], &dt_min, 8); memcpy(&key[5], &dt_max, 8);
     for (int k = 0; k < order && k < 4; ++k) key[20 + k] = (unsigned long long)(uintptr_t)a_derivs[k];
     for (int k = 4; k < order; ++k) key[20 + (k & 3)] ^= (unsigned long long)(uintptr_t)a_derivs[k] * 0x9e3779b97f4a7c15ull;
     if (c->use_graph && (!c->graph_exec || memcmp(key, c->graph_key, sizeof(key)) != 0)) {
-        if (c->graph_exec) {
-            cudaGraphExecDestroy(c->graph_exec);
-            c->graph_exec = nullptr;
+        for (cudaGraphExec_t *ge : {&c->graph_exec, &c->graph_small}) {
+            if (*ge) cudaGraphExecDestroy(*ge);
+            *ge = nullptr;
         }
-        cudaGraph_t graph = nullptr;
-        NB_CUDA(c, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-        const int rc = enqueue_step(st);
-        const cudaError_t e = cudaStreamEndCapture(st, &graph);
-        if (rc != NBODY_OK) {
-            if (graph) cudaGraphDestroy(graph);
-            return rc;
+        for (int which = 0; which < 2; ++which) {
+            cudaGraph_t graph = nullptr;
+            NB_CUDA(c, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int rc = which == 0 ? enqueue_step(st) : enqueue_fused(st);
+            const cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (rc != NBODY_OK) {
+                if (graph) cudaGraphDestroy(graph);
+                return rc;
+            }
+            NB_CUDA(c, e);
+            const cudaError_t ei = cudaGraphInstantiate(which == 0 ? &c->graph_exec : &c->graph_small, graph, 0);
+            cudaGraphDestroy(graph);
+            NB_CUDA(c, ei);
         }
-        NB_CUDA(c, e);
-        const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0);
-        cudaGraphDestroy(graph);
-        NB_CUDA(c, ei);
         memcpy(c->graph_key, key, sizeof(key));
     }
+    auto step = [&](bool small) -> int {
+        c->launches += small ? kFusedLaunches : kStepLaunches;
+        if (c->use_graph) {
+            const cudaError_t e = cudaGraphLaunch(small ? c->graph_small : c->graph_exec, st);
+            return e == cudaSuccess ? NBODY_OK : cuda_fail(c, e);
+        }
+        return small ? enqueue_fused(st) : enqueue_step(st);
+    };
 
-    // batches of block steps between two looks at the control block
+    // batches of block steps between two looks at the control block.  With the fused step on, runs of blocks that
+    // fit one i-tile go through it; a larger block stops such a batch (stop = 4) and is taken by the general step.
     int batch = 8;
     int rc = NBODY_OK;
     for (;;) {
-        for (int b = 0; b < batch && rc == NBODY_OK; ++b) {
-            if (c->use_graph) {
-                const cudaError_t e = cudaGraphLaunch(c->graph_exec, st);
-                if (e != cudaSuccess) rc = cuda_fail(c, e);
-            } else {
-                rc = enqueue_step(st);
-            }
-            c->launches += kStepLaunches;
-        }
+        for (int b = 0; b < batch && rc == NBODY_OK; ++b) rc = step(fused);
         if (rc != NBODY_OK) break;
         cudaError_t e = cudaMemcpyAsync(hc, c->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if (hc->stop == 4) {
+            e = cudaMemsetAsync(&c->d_ctl->stop, 0, sizeof(int), st);
+            if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
+            rc = step(false);
+            if (rc != NBODY_OK) break;
+            if (batch > 8) batch /= 2;
+            continue;
+        }
         if (hc->stop) break;
         if (batch < 64) batch *= 2;
     }
@@ -1115,6 +964,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     res->t_next = hc->t_next;
     res->n_act_next = (int64_t)hc->n_act;
     res->stop_reason = hc->stop;
+    res->rejected = (int64_t)hc->rejected;
     for (int b = 0; b < 40; ++b) res->hist_log2[b] = (int64_t)hc->hist[b];
     NB_CUDA(c, cudaEventRecord(h->ev_out, st));
     NB_CUDA(c, cudaStreamWaitEvent(user, h->ev_out, 0));

@@ -27,6 +27,7 @@
 //     (device-driven block step, nbody_run_blocks).
 #include <math.h>
 
+#include "nbody_exact.cuh"
 #include "nbody_internal.h"
 
 
@@ -510,14 +511,14 @@ __device__ __forceinline__ void reduce_store(double s, long long o, int nc, int 
 }
 
 __device__ __forceinline__ void reduce_body(const double *partials, int splits, int nc, int n_act, double *acc,
-                                            double *jerk, double *snap, double *crk, double *pot) {
+                                            double *jerk, double *snap, double *crk, double *pot, const long long tid,
+                                            const long long nthr) {
     const long long tot = (long long)nc * n_act;
-    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nthr = (long long)gridDim.x * blockDim.x;
     if (splits <= 8) {
         for (long long o = tid; o < tot; o += nthr) {
             double v[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) v[k] = k < splits ? partials[(size_t)k * tot + o] : 0.0;
+            for (int k = 0; k < 8; ++k) v[k] = k < splits ? __ldcg(partials + (size_t)k * tot + o) : 0.0;
             double s = v[0];
 #pragma unroll
             for (int k = 1; k < 8; ++k)
@@ -529,7 +530,7 @@ __device__ __forceinline__ void reduce_body(const double *partials, int splits, 
         for (long long o = tid >> 5; o < tot; o += nthr >> 5) {
             double s = 0.0;
 #pragma unroll 4
-            for (int k = lane; k < splits; k += 32) s += partials[(size_t)k * tot + o];
+            for (int k = lane; k < splits; k += 32) s += __ldcg(partials + (size_t)k * tot + o);
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
             if (lane == 0) reduce_store(s, o, nc, n_act, acc, jerk, snap, crk, pot);
@@ -539,13 +540,262 @@ __device__ __forceinline__ void reduce_body(const double *partials, int splits, 
 
 __global__ void __launch_bounds__(256) k_reduce(const double *partials, int splits, int nc, int n_act, double *acc,
                                                 double *jerk, double *snap, double *crk, double *pot) {
-    reduce_body(partials, splits, nc, n_act, acc, jerk, snap, crk, pot);
+    reduce_body(partials, splits, nc, n_act, acc, jerk, snap, crk, pot,
+                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
 __global__ void __launch_bounds__(256) k_reduce_dyn(const Ctl *ctl, const double *partials, int nc, double *acc,
                                                     double *jerk, double *snap, double *crk, double *pot) {
     if (ctl->stop || ctl->splits == 1) return;
-    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot);
+    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot,
+                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// N1 -- the fused small-block step ("real core-halo density structure ... block
+// time-steps": most block steps of such a system move a handful of particles).  For a block that fits one i-tile
+// (n_act <= 2 kThreads / JL, i.e. <= 1024) the j-store round trip is dropped: every persistent CTA owns one j-split,
+// pulls the RAW fp64 Taylor state of its j-tiles into shared memory by TMA (two stages), 256 of its threads run the
+// bit-exact Horner predictor (predict_particle, the code of K_pred) on one particle each and leave the packed quads of
+// the tile in shared memory, then all 512 threads run the ordinary pair loop on it.  Every j is predicted exactly
+// once in the whole grid; the i-particles are predicted by their own threads (the same arithmetic, so the self
+// differences are still exactly zero, R4).  The last CTA to finish sums the j-split partials (K_reduce's fixed tree)
+// and runs the corrector (correct_one, the code of K_corr) for the block: one launch instead of four.
+// Results are bit-identical to K_pred + K_force + K_reduce + K_corr.
+// ---------------------------------------------------------------------------------------------------------
+struct FusedArgs {
+    ForceArgs F;                    // idx, n, n_tiles, eps2, out, partials, ctl (q[] unused)
+    const double *t, *m, *x, *v;    // raw state: the predictor's inputs
+    const double *D[6];
+    CorrArgs C;                     // corrector arguments (control-block mode)
+    int tma_ok;                     // every raw array is 16-byte aligned: full tiles come in by TMA
+};
+
+template <int ORDER>
+struct FGeo {
+    static constexpr int K = ORDER / 2, NC = 3 * K + 1, ND = ORDER - 2;
+    static constexpr int NQ = ORDER == 4 ? 3 : 4;
+    static constexpr int RSTAGES = 2;
+    static constexpr uint32_t RAW_DOUBLES = kTileJ * (2 + 3 * (2 + ND));  // t, m, x[3], v[3], D_k[3]
+    static constexpr uint32_t RAW_BYTES = RAW_DOUBLES * 8;
+    static constexpr size_t PRED_BYTES = (size_t)NQ * kTileJ * 16;
+    static constexpr size_t ACC_BYTES = (size_t)2 * NC * kThreads * sizeof(double);
+    static constexpr size_t SMEM = RSTAGES * (size_t)RAW_BYTES + PRED_BYTES + ACC_BYTES + 128;
+};
+
+template <int ORDER, int JL>
+__device__ __forceinline__ void fused_item(const FusedArgs &A, const int n_act, const int splits, const int split,
+                                           const double t_now, unsigned char *smem_raw, unsigned &tile_run) {
+    typedef FGeo<ORDER> G;
+    constexpr int NC = G::NC, ND = G::ND, RST = G::RSTAGES;
+    constexpr int IT = kThreads / JL, JPT = kTileJ / JL;
+    double *raw = reinterpret_cast<double *>(smem_raw);
+    uint4 *pred = reinterpret_cast<uint4 *>(smem_raw + RST * (size_t)G::RAW_BYTES);
+    double *acc_sm = reinterpret_cast<double *>(smem_raw + RST * (size_t)G::RAW_BYTES + G::PRED_BYTES);
+    const uint32_t bar0 = smem_u32(smem_raw + RST * (size_t)G::RAW_BYTES + G::PRED_BYTES + G::ACC_BYTES);
+    const int tid = threadIdx.x;
+    const int il = JL == 1 ? tid : tid % IT, jl = JL == 1 ? 0 : tid / IT;
+    const ForceArgs &F = A.F;
+    const int tile_lo = (int)((long long)F.n_tiles * split / splits);
+    const int tile_hi = (int)((long long)F.n_tiles * (split + 1) / splits);
+    const int ntile = tile_hi - tile_lo;
+    // a tile comes in by TMA iff it is full and the arrays are aligned; only the last tile of the array can be ragged
+    auto by_tma = [&](int k) { return A.tma_ok && (tile_lo + k + 1) * kTileJ <= F.n; };
+    auto issue = [&](int k, unsigned g) {  // tile k of this item is TMA tile number g of this CTA
+        const int s = g % RST;
+        const uint32_t bar = bar0 + 8 * s;
+        mbar_expect_tx(bar, G::RAW_BYTES);
+        const size_t b = (size_t)(tile_lo + k) * kTileJ;
+        double *dst = raw + (size_t)s * G::RAW_DOUBLES;
+        bulk_g2s(smem_u32(dst), A.t + b, kTileJ * 8, bar);
+        bulk_g2s(smem_u32(dst + kTileJ), A.m + b, kTileJ * 8, bar);
+        bulk_g2s(smem_u32(dst + 2 * kTileJ), A.x + 3 * b, kTileJ * 24, bar);
+        bulk_g2s(smem_u32(dst + 5 * kTileJ), A.v + 3 * b, kTileJ * 24, bar);
+#pragma unroll
+        for (int d = 0; d < ND; ++d) bulk_g2s(smem_u32(dst + (8 + 3 * d) * kTileJ), A.D[d] + 3 * b, kTileJ * 24, bar);
+    };
+    unsigned g_issue = tile_run, g_use = tile_run;  // TMA tiles issued / consumed so far by this CTA
+    if (tid == 0 && ntile > 0 && by_tma(0)) issue(0, g_issue);
+    if (ntile > 0 && by_tma(0)) ++g_issue;
+
+    // ---- the thread's two i-particles: predicted here from the raw state (same arithmetic as for the j: R4) ----
+    IPair<ORDER, 0> I;
+    float nv[2][3], na[2][3], nj[2][3];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int slot = r * IT + il;
+        const bool valid = slot < n_act;
+        const long long gi = F.idx[valid ? slot : n_act - 1];
+        I.idx[r] = valid ? (int)gi : -1;
+        const double *Dp[6];
+#pragma unroll
+        for (int d = 0; d < ND; ++d) Dp[d] = A.D[d] + 3 * gi;
+        double xp[3];
+        float vp[3], ap[3], jp[3];
+        predict_particle<ORDER>(d_sub(t_now, A.t[gi]), A.x + 3 * gi, A.v + 3 * gi, Dp, xp, vp, ap, jp);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            I.x[r][c] = xp[c];
+            nv[r][c] = -vp[c];
+            na[r][c] = -ap[c];
+            nj[r][c] = -jp[c];
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        I.nv[c] = pk(nv[0][c], nv[1][c]);
+        if (ORDER >= 6) I.na[c] = pk(na[0][c], na[1][c]);
+        if (ORDER >= 8) I.nj[c] = pk(nj[0][c], nj[1][c]);
+    }
+    Consts C;
+    C.eps2 = pk(F.eps2, F.eps2);
+    C.m3 = pk(-3.f, -3.f);
+    C.three = pk(3.f, 3.f);
+    C.m4 = pk(-4.f, -4.f);
+    C.n = F.n;
+    f2 pa[NC];
+    double *acc_mine = acc_sm + tid;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        pa[c] = 0ull;
+        acc_mine[(2 * c) * kThreads] = 0.0;
+        acc_mine[(2 * c + 1) * kThreads] = 0.0;
+    }
+
+    int since = 0;
+#pragma unroll 1
+    for (int k = 0; k < ntile; ++k) {
+        const int j0 = (tile_lo + k) * kTileJ;
+        const bool tma_k = by_tma(k);
+        // producer: the raw data of tile k+1 goes into the other stage, which tile k-1's predictors have released
+        if (k + 1 < ntile && by_tma(k + 1)) {
+            if (tid == 0) {
+                if (g_issue >= RST)
+                    mbar_wait(bar0 + 8 * (RST + (g_issue - RST) % RST), (uint32_t)(((g_issue - RST) / RST) & 1));
+                issue(k + 1, g_issue);
+            }
+            ++g_issue;
+        }
+        // ---- predict phase: thread p < 256 predicts particle j0 + p into the packed tile ----
+        if (tid < kTileJ) {
+            const int p = tid;
+            double xp[3] = {kPadPos, kPadPos, kPadPos};
+            float vp[3] = {0.f, 0.f, 0.f}, ap[3] = {0.f, 0.f, 0.f}, jp[3] = {0.f, 0.f, 0.f}, m32 = 0.f;
+            if (tma_k) {
+                const int s = g_use % RST;
+                mbar_wait(bar0 + 8 * s, (uint32_t)((g_use / RST) & 1));
+                const double *st = raw + (size_t)s * G::RAW_DOUBLES;
+                const double *Dp[6];
+#pragma unroll
+                for (int d = 0; d < ND; ++d) Dp[d] = st + (8 + 3 * d) * kTileJ + 3 * p;
+                predict_particle<ORDER>(d_sub(t_now, st[p]), st + 2 * kTileJ + 3 * p, st + 5 * kTileJ + 3 * p, Dp, xp, vp,
+                                        ap, jp);
+                m32 = __double2float_rn(st[kTileJ + p]);
+                __syncwarp();
+                if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (RST + s));  // this warp is done with the raw stage
+            } else if (j0 + p < F.n) {  // ragged last tile / unaligned arrays: straight from global memory
+                const long long j = j0 + p;
+                const double *Dp[6];
+#pragma unroll
+                for (int d = 0; d < ND; ++d) Dp[d] = A.D[d] + 3 * j;
+                predict_particle<ORDER>(d_sub(t_now, A.t[j]), A.x + 3 * j, A.v + 3 * j, Dp, xp, vp, ap, jp);
+                m32 = __double2float_rn(A.m[j]);
+            }
+            pred[p] = pack_dd(xp[0], xp[1]);
+            pred[kTileJ + p] = pack_dff(xp[2], m32, vp[0]);
+            pred[2 * kTileJ + p] = pack_ffff(vp[1], vp[2], ap[0], ap[1]);
+            if (ORDER >= 6) pred[3 * kTileJ + p] = pack_ffff(ap[2], jp[0], jp[1], jp[2]);
+        }
+        if (tma_k) ++g_use;
+        __syncthreads();
+        // ---- pair loop on the predicted tile ----
+        const bool mine = (unsigned)(I.idx[0] - j0) < (unsigned)kTileJ || (unsigned)(I.idx[1] - j0) < (unsigned)kTileJ;
+        if (__any_sync(0xffffffffu, mine) || j0 + kTileJ > F.n)
+            tile_compute<ORDER, JL, 0, true>(I, pred, j0, jl, C, pa, acc_mine);
+        else
+            tile_compute<ORDER, JL, 0, false>(I, pred, j0, jl, C, pa, acc_mine);
+        if (JPT < 64) {
+            if (++since == 64 / JPT) {
+                since = 0;
+                flush(pa, acc_mine);
+            }
+        }
+        __syncthreads();  // the tile buffer is free for the next predict phase
+    }
+    tile_run = g_use;
+    flush(pa, acc_mine);
+    __syncthreads();
+
+    // ---- epilogue: fixed-order sum over the JL j-lanes, pot = - Sum m/r (as force_item, i-tile 0) ----
+    for (int o = tid; o < 2 * IT * NC; o += kThreads) {
+        const int comp = o / (2 * IT), rem = o % (2 * IT);
+        const int r = rem / IT, i_l = rem % IT;
+        double sum = 0.0;
+#pragma unroll 8
+        for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
+        const int slot = r * IT + i_l;
+        if (slot < n_act) {
+            if (comp == NC - 1) sum = -sum;
+            if (splits == 1) {
+                if (comp == NC - 1) F.out[4][slot] = sum;
+                else F.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
+            } else {
+                F.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+            }
+        }
+    }
+}
+
+template <int ORDER>
+__global__ void __launch_bounds__(kThreads, 1) k_step_fused(const FusedArgs A) {
+    typedef FGeo<ORDER> G;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ int s_last;
+    Ctl *ctl = const_cast<Ctl *>(A.F.ctl);
+    if (ctl->stop || ctl->i_tiles != 1) return;  // (the selection stops a fused run in front of a larger block)
+    const int n_act = (int)ctl->n_act, jl = ctl->jl, splits = ctl->splits;
+    const double t_now = ctl->t_next;
+    const int tid = threadIdx.x;
+    const uint32_t bar0 = smem_u32(smem_raw + G::RSTAGES * (size_t)G::RAW_BYTES + G::PRED_BYTES + G::ACC_BYTES);
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < G::RSTAGES; ++s) {
+            mbar_init(bar0 + 8 * s, 1);                              // full[s]: the TMA transaction
+            mbar_init(bar0 + 8 * (G::RSTAGES + s), kTileJ / 32);     // empty[s]: one arrival per predicting warp
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    unsigned tile_run = 0;
+    for (int w = blockIdx.x; w < splits; w += gridDim.x) {
+        switch (jl) {
+            case 1: fused_item<ORDER, 1>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 2: fused_item<ORDER, 2>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 4: fused_item<ORDER, 4>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 8: fused_item<ORDER, 8>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 32: fused_item<ORDER, 32>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            default: fused_item<ORDER, 128>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+        }
+        __syncthreads();
+    }
+    // ---- the last CTA to get here sums the split partials and corrects the block ----
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned ticket = atomicAdd(&ctl->tickets[0], 1u);
+        s_last = ticket == gridDim.x - 1;
+        if (s_last) ctl->tickets[0] = 0;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const ForceArgs &F = A.F;
+    if (splits > 1) {
+        reduce_body(F.partials, splits, G::NC, n_act, F.out[0], F.out[1], F.out[2], F.out[3], F.out[4], tid, kThreads);
+        __threadfence_block();
+        __syncthreads();
+    }
+    for (long long ia = tid; ia < n_act; ia += kThreads) correct_one<ORDER>(A.C, ia, t_now);
 }
 
 typedef void (*force_fn)(const ForceArgs);
@@ -613,6 +863,29 @@ int force_static_init(Ctx *c) {
         NB_CUDA(c, cudaFuncSetAttribute((const void *)pick_dyn(orders[o]), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)smem_for(orders[o], 0)));
     }
+    NB_CUDA(c, cudaFuncSetAttribute((const void *)k_step_fused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FGeo<4>::SMEM));
+    NB_CUDA(c, cudaFuncSetAttribute((const void *)k_step_fused<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FGeo<6>::SMEM));
+    NB_CUDA(c, cudaFuncSetAttribute((const void *)k_step_fused<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FGeo<8>::SMEM));
+    return NBODY_OK;
+}
+
+int launch_step_fused(Ctx *c, int order, float eps2, const int32_t *active_idx, const double *t, const double *m,
+                      const double *x, const double *v, const double *const a_derivs[8], const CorrArgs &corr,
+                      double *acc, double *jerk, double *snap, double *crackle, double *pot, cudaStream_t st) {
+    FusedArgs A;
+    fill_args(c, A.F, active_idx, eps2, acc, jerk, snap, crackle, pot);
+    A.t = t; A.m = m; A.x = x; A.v = v;
+    bool aligned = ((uintptr_t)t | (uintptr_t)m | (uintptr_t)x | (uintptr_t)v) % 16 == 0;
+    for (int k = 0; k < 6; ++k) {
+        A.D[k] = k <= order - 3 ? a_derivs[k] : nullptr;
+        if (A.D[k] && (uintptr_t)A.D[k] % 16 != 0) aligned = false;
+    }
+    A.C = corr;
+    A.tma_ok = aligned ? 1 : 0;
+    if (order == 4) k_step_fused<4><<<c->sm_count, kThreads, FGeo<4>::SMEM, st>>>(A);
+    else if (order == 6) k_step_fused<6><<<c->sm_count, kThreads, FGeo<6>::SMEM, st>>>(A);
+    else k_step_fused<8><<<c->sm_count, kThreads, FGeo<8>::SMEM, st>>>(A);
+    NB_CUDA(c, cudaGetLastError());
     return NBODY_OK;
 }
 

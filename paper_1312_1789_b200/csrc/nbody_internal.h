@@ -88,6 +88,7 @@ struct Ctl {
     int error;                    // validation failure code (device-side checks)
     int jl, splits;               // force geometry of the current block (force_geometry(), evaluated on the device)
     long long i_tiles;
+    unsigned long long rejected;  // steps refused by the a-posteriori rule (R14) since the counter was last reset
     unsigned int tickets[4];      // last-CTA tickets
     unsigned long long hist[40];  // executed blocks by floor(log2 n_act)
 };
@@ -116,7 +117,8 @@ struct Ctx {
     void *stage = nullptr;
     size_t stage_bytes = 0;
     // block-step graph cache (nbody_run_blocks)
-    cudaGraphExec_t graph_exec = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;        // general step: select, predict, force, reduce, correct
+    cudaGraphExec_t graph_small = nullptr;       // fused small-block step (N1): select, fused step
     unsigned long long graph_key[24] = {0};
     // options
     int diff_mode = 0;
@@ -126,6 +128,8 @@ struct Ctx {
     int crit_order = 0;  // 0 = automatic (4 for p >= 6, else p); 4 | 6 | 8 = criterion order min(p, value) (R8 / R8b)
     int validate = 0;
     int use_graph = 1;
+    int use_fused = 1;     // N1: runs of blocks that fit one i-tile go through the fused step
+    int reject_ratio = 0;  // R14: 0 = off; R = 2^r >= 2: a step whose end-point criterion asks for dt <= h/R is refused
     // bookkeeping
     int last_cuda_error = 0;
     int64_t launches = 0;
@@ -179,6 +183,11 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
 int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, double *acc, double *jerk, double *snap,
                      double *crackle, double *pot, cudaStream_t st);
 int force_static_init(Ctx *c);
+struct CorrArgs;
+// N1: predict + force + reduce + correct of a block that fits one i-tile, in one launch (reads the control block)
+int launch_step_fused(Ctx *c, int order, float eps2, const int32_t *active_idx, const double *t, const double *m,
+                      const double *x, const double *v, const double *const a_derivs[8], const CorrArgs &corr,
+                      double *acc, double *jerk, double *snap, double *crackle, double *pot, cudaStream_t st);
 // implemented in nbody_probe.cu
 int probe_peak(Ctx *c, int kind, int millis, double *tera_ops);
 

@@ -30,16 +30,21 @@ def _same_state(a, b, order):
         assert np.array_equal(a.D[k].cpu().numpy(), b.D[k].cpu().numpy()), "a^(%d)" % k
 
 
-@pytest.mark.parametrize("order,use_graph", [(4, 1), (6, 1), (8, 1), (6, 0)])
-def test_run_blocks_bit_identical_to_host_driven_path(order, use_graph):
+@pytest.mark.parametrize("order,use_graph,use_fused,n", [(4, 1, 1, 3001), (6, 1, 1, 3001), (8, 1, 1, 3001), (6, 0, 1, 3001),
+                                                         (6, 1, 0, 3001), (8, 1, 1, 4096), (4, 0, 0, 2048)])
+def test_run_blocks_bit_identical_to_host_driven_path(order, use_graph, use_fused, n):
+    """use_fused = 1: blocks that fit one i-tile go through the fused step (N1: predict-in-force + last-CTA reduce and
+    correct, raw state by TMA; n = 3001 also exercises the ragged last tile, n = 4096 all-TMA tiles), larger blocks
+    through the general graph; use_fused = 0: every block through the general graph."""
     import torch
     K = 150
-    c, a, b = _pair(5, 3001, order, dt_max=2.0**-5)
+    c, a, b = _pair(5, n, order, dt_max=2.0**-5)
     sizes = []
     for _ in range(K):
         _, na = a.block_step()
         sizes.append(na)
     b.ctx.set_option("use_graph", use_graph)
+    b.ctx.set_option("use_fused", use_fused)
     r = b.run(1.0, max_blocks=K)
     torch.cuda.synchronize()
     assert r["blocks"] == K and r["stop_reason"] == 3
@@ -48,12 +53,35 @@ def test_run_blocks_bit_identical_to_host_driven_path(order, use_graph):
     for s in sizes:
         hist[int(s).bit_length() - 1] += 1
     assert r["hist_log2"] == hist
-    assert len(set(sizes)) > 5 and max(sizes) > 64 and min(sizes) < 8  # every lane variant / split is exercised
+    assert len(set(sizes)) > 5 and max(sizes) > 1024 and min(sizes) < 8  # every lane variant, both step flavours
     _same_state(a, b, order)
     # the block that stopped the run is the next block of the host-driven path
     tn, na = a.ctx.next_block(a.n, a.t, a.dt, a.active)
     assert r["t_next"] == tn and r["n_act_next"] == na
     assert np.array_equal(a.active[:na].cpu().numpy(), b.active[:na].cpu().numpy())
+
+
+def test_fused_step_with_unaligned_state_arrays():
+    """State arrays that are only 8-byte aligned cannot come in by TMA bulk copies (16-byte rule): the fused step reads
+    them with plain loads instead; results stay bit-identical."""
+    import torch
+    order = 6
+    c, a, b = _pair(3, 2048, order, dt_max=2.0**-6)
+
+    def shifted(tn):
+        flat = torch.zeros(tn.numel() + 1, dtype=torch.float64, device="cuda")
+        view = flat[1:].view(tn.shape)
+        view.copy_(tn)
+        assert view.data_ptr() % 16 == 8
+        return view
+
+    b.x, b.v, b.t = shifted(b.x), shifted(b.v), shifted(b.t)
+    b.D = [shifted(d) for d in b.D]
+    for _ in range(60):
+        a.block_step()
+    r = b.run(1.0, max_blocks=60)
+    assert r["blocks"] == 60
+    _same_state(a, b, order)
 
 
 def test_run_blocks_stop_reasons_and_resume():

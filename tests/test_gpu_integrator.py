@@ -246,3 +246,73 @@ def test_force_host_matches_device_path(nb, O):
     ref = O.force(c["m"], xp, vp, ap, jp, idx, order, c["eps2"])
     U.check_force((acc, jerk, snap, None, pot), ref, order, "force_host")
     ctx.close()
+
+
+def test_correct_step_rejection_bit_exact(nb, O):
+    """R14 (oracle c-9b): with a small eta many end-point criteria ask for dt <= h/4; those particles must keep their
+    whole state except dt = h/4, bit for bit as in the oracle, and the device counter equals the oracle's count."""
+    import torch
+    n, order = 3001, 8
+    c, D, t, dt = _state(3, n, order)
+    t_now = 2.0**-10
+    idx = W.active_list(n, 1500, W.rng_for(3, 22))
+    xp, vp, ap, jp = O.predict(t_now, order, t, c["x"], c["v"], D)
+    f = O.force(c["m"], xp, vp, ap, jp, idx, order, c["eps2"])
+    for R, eta in ((4, 0.004), (2, 0.02), (16, 0.001)):
+        ot, odt, ox, ov, oD, op = t.copy(), dt.copy(), c["x"].copy(), c["v"].copy(), [d.copy() for d in D], np.zeros(n)
+        nrej = O.correct(idx, order, t_now, eta, 2.0**-30, 2.0**-4, ot, odt, ox, ov, oD, op, *f, reject_ratio=R)
+        assert 0 < nrej < idx.shape[0]
+        ctx = nb.Context(n)
+        ctx.set_option("step_reject_ratio", R)
+        gt, gdt, gx, gv, gD, gp = U.dev(t), U.dev(dt), U.dev(c["x"]), U.dev(c["v"]), [U.dev(d) for d in D], U.zeros(n)
+        ctx.correct(U.dev(idx), idx.shape[0], order, t_now, eta, 2.0**-30, 2.0**-4, gt, gdt, gx, gv, gD, gp,
+                    *[U.dev(a) for a in f])
+        assert ctx.rejected_steps(reset=True) == nrej and ctx.rejected_steps() == 0
+        for a, b in ((gt, ot), (gdt, odt), (gx, ox), (gv, ov), (gp, op)):
+            assert np.array_equal(a.cpu().numpy(), b)
+        for k in range(8):
+            assert np.array_equal(gD[k].cpu().numpy(), oD[k])
+        rej = idx[ot[idx] != t_now]
+        assert rej.shape[0] == nrej and np.all(odt[rej] == dt[rej] / R)
+        ctx.close()
+    with pytest.raises(nb.NBodyError):
+        nb.Context(4).set_option("step_reject_ratio", 3)
+
+
+@pytest.mark.parametrize("order", [6, 8])
+def test_flyby_step_rejection_gpu(nb, order):
+    """The oracle's fly-by pin on the CUDA path (closest approach on the end point of a long first step): without R14
+    the energy error is astronomic, with step_reject_ratio = 4 the step is refused and redone on shorter steps --
+    through block times that run BACKWARDS for the refused particles -- and the device-driven run reproduces the
+    host-driven one bit for bit."""
+    import torch
+    from paper_1312_1789_b200.scheduler import Integrator
+    h0 = 2.0**-4
+    m = np.array([5e-4, 5e-4])
+    x = np.array([[-h0 / 2, 5e-4, 0.0], [h0 / 2, -5e-4, 0.0]])
+    v = np.array([[0.5, 0.0, 0.0], [-0.5, 0.0, 0.0]])
+
+    def energy(g):
+        xx, vv = g.x.cpu().numpy(), g.v.cpu().numpy()
+        return 0.5 * np.sum(m * np.sum(vv * vv, axis=1)) - m[0] * m[1] / np.linalg.norm(xx[0] - xx[1])
+
+    out = {}
+    for R, driver in ((0, "host"), (4, "host"), (4, "device")):
+        g = Integrator(m, x, v, order, 0.0, dt_min=2.0**-40, dt_max=h0, step_reject_ratio=R)
+        g.bootstrap(fixed_dt=h0)
+        e0 = energy(g)
+        if driver == "host":
+            g.integrate(2 * h0)
+            rej = g.ctx.rejected_steps()
+        else:
+            r = g.run(2 * h0)
+            rej = r["rejected"]
+        torch.cuda.synchronize()
+        assert bool((g.t == 2 * h0).all())
+        out[(R, driver)] = (abs((energy(g) - e0) / e0), rej, g.blocks, g.x.cpu().numpy(), g.v.cpu().numpy())
+    assert out[(0, "host")][0] > 1e3 and out[(0, "host")][1] == 0
+    assert out[(4, "host")][0] < 1e-5 and out[(4, "host")][1] >= 1
+    a, b = out[(4, "host")], out[(4, "device")]
+    assert a[1] == b[1] and a[2] == b[2] and np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
+    ang = np.degrees(np.arctan2(a[4][0][1], a[4][0][0]))
+    assert abs(abs(ang) - 90.0) < 2.5

@@ -536,3 +536,63 @@ def test_block_timestep_energy_conservation_criterion_order4():
     assert np.all(s.t == 0.125)
     e1 = OI.total_energy(s, eps2)
     assert abs((e1 - e0) / e0) < 1e-7
+
+
+# ------------------------------------------------------------------------------------------- c-9b (R14)
+def _flyby(order, reject_ratio, h0=2.0**-4):
+    """Two equal masses (M = 1e-3) on a hyperbolic orbit, impact parameter b = 1e-3, v_inf = 1: closest approach
+    (r_min = 4.1e-4) falls on the END of the first step h0 = 2^-4 that both particles are started with."""
+    m = np.array([5e-4, 5e-4])
+    b = 1e-3
+    x = np.array([[-h0 / 2, b / 2, 0.0], [h0 / 2, -b / 2, 0.0]])
+    v = np.array([[0.5, 0.0, 0.0], [-0.5, 0.0, 0.0]])
+    s = OI.bootstrap(m, x, v, order, 0.0, fixed_dt=h0, dt_min=2.0**-40, dt_max=h0)
+    e0 = _energy2(s.m, s.x, s.v)
+    l0 = np.sum(s.m[:, None] * np.cross(s.x, s.v), axis=0)[2]
+    nb, _ = OI.integrate(s, 2 * h0, 0.0, 0.1, 2.0**-40, h0, reject_ratio=reject_ratio)
+    assert np.all(s.t == 2 * h0)
+    e1 = _energy2(s.m, s.x, s.v)
+    l1 = np.sum(s.m[:, None] * np.cross(s.x, s.v), axis=0)[2]
+    return abs((e1 - e0) / e0), abs((l1 - l0) / l0), s, nb
+
+
+@pytest.mark.parametrize("order", [4, 6, 8])
+def test_step_rejection_flyby_pin(order):
+    """c-9b against the two-body invariants and the closed-form deflection: an encounter whose closest approach sits on
+    the end point of a long step wrecks the textbook scheme (the end-point derivatives m v^k / r^(k+2) are extrapolated
+    over the whole step: |dE/E| > 1e4), while with reject_ratio = 4 the step is refused, redone on h/4, and energy and
+    angular momentum are conserved; the velocity turns by theta = 2 atan(M / (b v_inf^2)) = 90 degrees."""
+    bad_e, bad_l, _, _ = _flyby(order, 0)
+    good_e, good_l, s, nb = _flyby(order, 4)
+    assert bad_e > 1e3
+    assert good_e < {4: 1e-6, 6: 1e-9, 8: 1e-10}[order] and good_l < {4: 1e-6, 6: 1e-9, 8: 1e-10}[order]
+    assert s.rejected >= 1 and nb > 100
+    ang = math.degrees(math.atan2(s.v[0][1], s.v[0][0]))  # started along +x
+    assert abs(abs(ang) - 90.0) < 2.5, ang  # asymptotic value 90; the run ends 0.06 = 60 b after the pericentre
+    assert abs(np.linalg.norm(s.v[0] - s.v[1]) - 1.0) < 0.02  # |v_rel| back to v_inf (up to the residual potential)
+
+
+def test_step_rejection_rule_details():
+    """c-9b mechanics: a rejected particle keeps x, v, D, pot, t and only gets dt = h/R; the rule never fires when it
+    is off, when dt_new > h/R, or when h/R would fall below dt_min."""
+    n = 3
+    idx = np.arange(n, dtype=np.int32)
+    h = 2.0**-6
+    ex = np.array([1.0, 0.0, 0.0])
+    lam = np.array([1.0, 2.0**9, 2.0**9])  # particle 0: smooth; 1 and 2: dt_crit = eta / lam = 2^-3 / 2^9 = 2^-12
+    f = [np.ascontiguousarray(np.outer(lam**k * np.exp(lam * h), ex)) for k in range(2)]  # a(t) = e^(lam t)
+    mk = lambda: dict(t=np.zeros(n), dt=np.full(n, h), x=np.ones((n, 3)), v=np.ones((n, 3)),
+                      D=[np.ascontiguousarray(np.outer(lam**k, ex)) for k in range(8)], pot=np.zeros(n))
+    for R, dtmin, expect in ((0, 2.0**-30, [False, False, False]), (4, 2.0**-30, [False, True, True]),
+                             (4, 2.0**-7, [False, False, False]), (2.0**7, 2.0**-30, [False, False, False])):
+        s = mk()
+        ref = mk()
+        nrej = O.correct(idx, 4, h, 0.125, dtmin, 2.0**-2, s["t"], s["dt"], s["x"], s["v"], s["D"], s["pot"], f[0], f[1],
+                         None, None, np.full(n, -1.0), crit_order=4, reject_ratio=int(R))
+        assert nrej == sum(expect)
+        for i in range(n):
+            if expect[i]:
+                assert s["t"][i] == 0.0 and s["dt"][i] == h / R and s["pot"][i] == 0.0
+                assert np.array_equal(s["x"][i], ref["x"][i]) and np.array_equal(s["D"][2][i], ref["D"][2][i])
+            else:
+                assert s["t"][i] == h and s["pot"][i] == -1.0
