@@ -84,7 +84,14 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *   "validate"    0 = off [default]; 1 = debug mode: nbody_force checks on the device that active_idx is strictly
  *                 ascending (hence unique) and in [0, n), nbody_correct additionally that t[i] + dt[i] == t_now for
  *                 every active i; a violation returns NBODY_EINVAL before any arithmetic.  Synchronises `stream`.
- *   "use_graph"   1 = nbody_run_blocks replays its five launches as one CUDA graph [default]; 0 = plain launches
+ *   "use_graph"   1 = nbody_run_blocks replays its launches as CUDA graphs [default]; 0 = plain launches
+ *   "use_fused"   N1, fused small-block step.  0 [default] = every block of a run goes through the general step (five
+ *                 launches: selection, predictor, force, reduce, corrector).  1 = blocks that fit one i-tile (n_act <=
+ *                 1024) go through TWO launches: selection + a persistent kernel whose CTAs predict their j-tiles on the
+ *                 fly from the raw fp64 state (TMA-staged; the bit-exact predictor arithmetic) before the pair loop, and
+ *                 whose last CTA sums the j-split partials and runs the corrector; a larger block ends such a batch and is
+ *                 taken by the general step.  Bit-identical results either way.  Off by default because it is not yet
+ *                 faster (profiles/r02_latency.md: one 53 KB raw stage in flight per SM is latency-bound).
  *   "step_reject_ratio" R14, a-posteriori step rejection (a reading added by this build; the paper is silent):
  *                 0 = off [default], the textbook scheme.  R = 2^r in [2, 2^20]: if the criterion evaluated at the END of
  *                 a particle's step asks for dt_new <= h/R and h/R >= dt_min, nbody_correct does not take the step: x, v,

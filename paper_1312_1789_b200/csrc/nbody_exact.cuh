@@ -41,7 +41,9 @@ __device__ __forceinline__ uint4 pack_ffff(float a, float b, float c, float d) {
 
 // R5 for one particle: tau = t_now - t_i; x3, v3 and Dp[k] point at the particle's three components of x, v and
 // a^(k) (k = 0 .. ORDER-3).  Horner, innermost first, c_k = tau / k.  Outputs: x_p (fp64), v_p, a_p, j_p rounded to fp32.
-template <int ORDER>
+// The four polynomials are independent chains; DO_X .. DO_J select which of them this thread evaluates (the fused
+// small-block kernel splits a particle over two threads), the arithmetic of each is the same whoever evaluates it.
+template <int ORDER, bool DO_X = true, bool DO_V = true, bool DO_A = true, bool DO_J = true>
 __device__ __forceinline__ void predict_particle(const double tau, const double *x3, const double *v3,
                                                  const double *const *Dp, double (&xp)[3], float (&vp)[3],
                                                  float (&ap)[3], float (&jp)[3]) {
@@ -54,28 +56,36 @@ __device__ __forceinline__ void predict_particle(const double tau, const double 
         double Dk[ND];
 #pragma unroll
         for (int k = 0; k < ND; ++k) Dk[k] = Dp[k][d];
-        double s = Dk[ND - 1];
-#pragma unroll
-        for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k + 2], s));
-        const double vq = v3[d];
-        xp[d] = d_add(x3[d], d_mul(tau, d_add(vq, d_mul(c[2], s))));
-        s = Dk[ND - 1];
-#pragma unroll
-        for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k + 1], s));
-        vp[d] = __double2float_rn(d_add(vq, d_mul(tau, s)));
-        ap[d] = 0.f;
-        jp[d] = 0.f;
-        if (ORDER >= 6) {
+        double s;
+        if (DO_X) {
             s = Dk[ND - 1];
 #pragma unroll
-            for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k], s));
-            ap[d] = __double2float_rn(s);
+            for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k + 2], s));
+            xp[d] = d_add(x3[d], d_mul(tau, d_add(v3[d], d_mul(c[2], s))));
         }
-        if (ORDER >= 8) {
+        if (DO_V) {
             s = Dk[ND - 1];
 #pragma unroll
-            for (int k = ND - 1; k >= 2; --k) s = d_add(Dk[k - 1], d_mul(c[k - 1], s));
-            jp[d] = __double2float_rn(s);
+            for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k + 1], s));
+            vp[d] = __double2float_rn(d_add(v3[d], d_mul(tau, s)));
+        }
+        if (DO_A) {
+            ap[d] = 0.f;
+            if (ORDER >= 6) {
+                s = Dk[ND - 1];
+#pragma unroll
+                for (int k = ND - 1; k >= 1; --k) s = d_add(Dk[k - 1], d_mul(c[k], s));
+                ap[d] = __double2float_rn(s);
+            }
+        }
+        if (DO_J) {
+            jp[d] = 0.f;
+            if (ORDER >= 8) {
+                s = Dk[ND - 1];
+#pragma unroll
+                for (int k = ND - 1; k >= 2; --k) s = d_add(Dk[k - 1], d_mul(c[k - 1], s));
+                jp[d] = __double2float_rn(s);
+            }
         }
     }
 }

@@ -555,9 +555,9 @@ __global__ void __launch_bounds__(256) k_reduce_dyn(const Ctl *ctl, const double
 // N1 -- the fused small-block step ("real core-halo density structure ... block
 // time-steps": most block steps of such a system move a handful of particles).  For a block that fits one i-tile
 // (n_act <= 2 kThreads / JL, i.e. <= 1024) the j-store round trip is dropped: every persistent CTA owns one j-split,
-// pulls the RAW fp64 Taylor state of its j-tiles into shared memory by TMA (two stages), 256 of its threads run the
-// bit-exact Horner predictor (predict_particle, the code of K_pred) on one particle each and leave the packed quads of
-// the tile in shared memory, then all 512 threads run the ordinary pair loop on it.  Every j is predicted exactly
+// pulls the RAW fp64 Taylor state of its j-tiles into shared memory by TMA (two stages), its threads run the bit-exact
+// Horner predictor (predict_particle, the code of K_pred; two threads per particle, each its own polynomials) and leave
+// the packed quads of the tile in shared memory, then all 512 threads run the ordinary pair loop on it.  Every j is predicted exactly
 // once in the whole grid; the i-particles are predicted by their own threads (the same arithmetic, so the self
 // differences are still exactly zero, R4).  The last CTA to finish sums the j-split partials (K_reduce's fixed tree)
 // and runs the corrector (correct_one, the code of K_corr) for the block: one launch instead of four.
@@ -676,35 +676,51 @@ __device__ __forceinline__ void fused_item(const FusedArgs &A, const int n_act, 
             }
             ++g_issue;
         }
-        // ---- predict phase: thread p < 256 predicts particle j0 + p into the packed tile ----
-        if (tid < kTileJ) {
-            const int p = tid;
-            double xp[3] = {kPadPos, kPadPos, kPadPos};
-            float vp[3] = {0.f, 0.f, 0.f}, ap[3] = {0.f, 0.f, 0.f}, jp[3] = {0.f, 0.f, 0.f}, m32 = 0.f;
+        // ---- predict phase: particle j0 + p is predicted by TWO threads (warps 0-7: x_p and j_p, warps 8-15: v_p, a_p
+        //      and the mass), each writing its own bytes of the packed tile ----
+        {
+            const int p = tid & (kTileJ - 1), part = tid / kTileJ;
+            const bool real = j0 + p < F.n;
+            const double *st = nullptr;
             if (tma_k) {
                 const int s = g_use % RST;
                 mbar_wait(bar0 + 8 * s, (uint32_t)((g_use / RST) & 1));
-                const double *st = raw + (size_t)s * G::RAW_DOUBLES;
-                const double *Dp[6];
-#pragma unroll
-                for (int d = 0; d < ND; ++d) Dp[d] = st + (8 + 3 * d) * kTileJ + 3 * p;
-                predict_particle<ORDER>(d_sub(t_now, st[p]), st + 2 * kTileJ + 3 * p, st + 5 * kTileJ + 3 * p, Dp, xp, vp,
-                                        ap, jp);
-                m32 = __double2float_rn(st[kTileJ + p]);
-                __syncwarp();
-                if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (RST + s));  // this warp is done with the raw stage
-            } else if (j0 + p < F.n) {  // ragged last tile / unaligned arrays: straight from global memory
-                const long long j = j0 + p;
-                const double *Dp[6];
-#pragma unroll
-                for (int d = 0; d < ND; ++d) Dp[d] = A.D[d] + 3 * j;
-                predict_particle<ORDER>(d_sub(t_now, A.t[j]), A.x + 3 * j, A.v + 3 * j, Dp, xp, vp, ap, jp);
-                m32 = __double2float_rn(A.m[j]);
+                st = raw + (size_t)s * G::RAW_DOUBLES;
             }
-            pred[p] = pack_dd(xp[0], xp[1]);
-            pred[kTileJ + p] = pack_dff(xp[2], m32, vp[0]);
-            pred[2 * kTileJ + p] = pack_ffff(vp[1], vp[2], ap[0], ap[1]);
-            if (ORDER >= 6) pred[3 * kTileJ + p] = pack_ffff(ap[2], jp[0], jp[1], jp[2]);
+            // the particle's raw state: shared memory (TMA tile) or global memory (ragged last tile / unaligned arrays)
+            const double *tp = tma_k ? st + p : A.t + (j0 + p);
+            const double *mp = tma_k ? st + kTileJ + p : A.m + (j0 + p);
+            const double *xq = tma_k ? st + 2 * kTileJ + 3 * p : A.x + 3 * (size_t)(j0 + p);
+            const double *vq = tma_k ? st + 5 * kTileJ + 3 * p : A.v + 3 * (size_t)(j0 + p);
+            const double *Dp[6];
+#pragma unroll
+            for (int d = 0; d < ND; ++d) Dp[d] = tma_k ? st + (8 + 3 * d) * kTileJ + 3 * p : A.D[d] + 3 * (size_t)(j0 + p);
+            double xp[3] = {kPadPos, kPadPos, kPadPos};
+            float vp[3] = {0.f, 0.f, 0.f}, ap[3] = {0.f, 0.f, 0.f}, jp[3] = {0.f, 0.f, 0.f}, m32 = 0.f;
+            unsigned *w = reinterpret_cast<unsigned *>(pred);  // word view: quad q of plane P at w[4 * (P * kTileJ + q)]
+            if (part == 0) {
+                if (real) predict_particle<ORDER, true, false, false, true>(d_sub(t_now, *tp), xq, vq, Dp, xp, vp, ap, jp);
+                pred[p] = pack_dd(xp[0], xp[1]);
+                *reinterpret_cast<double *>(w + 4 * (kTileJ + p)) = xp[2];
+                if (ORDER >= 6) {
+                    w[4 * (3 * kTileJ + p) + 1] = __float_as_uint(jp[0]);
+                    w[4 * (3 * kTileJ + p) + 2] = __float_as_uint(jp[1]);
+                    w[4 * (3 * kTileJ + p) + 3] = __float_as_uint(jp[2]);
+                }
+            } else {
+                if (real) {
+                    predict_particle<ORDER, false, true, true, false>(d_sub(t_now, *tp), xq, vq, Dp, xp, vp, ap, jp);
+                    m32 = __double2float_rn(*mp);
+                }
+                w[4 * (kTileJ + p) + 2] = __float_as_uint(m32);
+                w[4 * (kTileJ + p) + 3] = __float_as_uint(vp[0]);
+                pred[2 * kTileJ + p] = pack_ffff(vp[1], vp[2], ap[0], ap[1]);
+                if (ORDER >= 6) w[4 * (3 * kTileJ + p)] = __float_as_uint(ap[2]);
+            }
+            if (tma_k) {
+                __syncwarp();
+                if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (RST + (g_use % RST)));  // this warp is done with the raw stage
+            }
         }
         if (tma_k) ++g_use;
         __syncthreads();
@@ -761,7 +777,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_step_fused(const FusedArgs A) {
 #pragma unroll
         for (int s = 0; s < G::RSTAGES; ++s) {
             mbar_init(bar0 + 8 * s, 1);                              // full[s]: the TMA transaction
-            mbar_init(bar0 + 8 * (G::RSTAGES + s), kTileJ / 32);     // empty[s]: one arrival per predicting warp
+            mbar_init(bar0 + 8 * (G::RSTAGES + s), kThreads / 32);   // empty[s]: one arrival per warp
         }
         mbar_fence_init();
     }

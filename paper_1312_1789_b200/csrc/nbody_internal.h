@@ -128,7 +128,7 @@ struct Ctx {
     int crit_order = 0;  // 0 = automatic (4 for p >= 6, else p); 4 | 6 | 8 = criterion order min(p, value) (R8 / R8b)
     int validate = 0;
     int use_graph = 1;
-    int use_fused = 1;     // N1: runs of blocks that fit one i-tile go through the fused step
+    int use_fused = 0;     // N1: 1 = runs of blocks that fit one i-tile go through the fused step (measured no faster yet)
     int reject_ratio = 0;  // R14: 0 = off; R = 2^r >= 2: a step whose end-point criterion asks for dt <= h/R is refused
     // bookkeeping
     int last_cuda_error = 0;
