@@ -45,28 +45,44 @@ def bootstrap(m, x, v, order, eps2, eta_s=0.01, dt_min=2.0**-30, dt_max=2.0**-4,
     return s
 
 
-def block_step(s, eps2, eta, dt_min, dt_max, variant=0, crit_order=0, reject_ratio=0):
+def block_step(s, eps2, eta, dt_min, dt_max, variant=0, crit_order=0, reject_ratio=0, n_iter=1):
     """One block step (a-1 .. a-4).  Returns (t_next, active_idx).  With reject_ratio (c-9b) a rejected particle stays at
-    its old time with a shorter step, so the next block time can lie before this one; s.rejected counts them."""
+    its old time with a shorter step, so the next block time can lie before this one; s.rejected counts them.
+
+    n_iter > 1 = P(EC)^n (the paper is silent): after the corrector, the active
+    particles' corrected x1, v1 and their new a1, j1 (the first evaluation) stand in for their predicted values, the
+    force on them is evaluated again, and the corrector is applied again FROM THE OLD STATE at t0 with the new force --
+    n evaluations in all.  n -> infinity converges to the implicit (time-symmetric for a shared constant step) Hermite
+    scheme."""
     p = s.order
     t_next, idx = O.next_block(s.t, s.dt)
-    xp, vp, ap, jp = O.predict(t_next, p, s.t, s.x, s.v, s.D)
-    acc, jerk, snap, crk, pot = O.force(s.m, xp, vp, ap, jp, idx, p, eps2)
-    s.rejected = getattr(s, "rejected", 0) + O.correct(idx, p, t_next, eta, dt_min, dt_max, s.t, s.dt, s.x, s.v, s.D,
-                                                        s.pot, acc, jerk, snap, crk, pot, variant=variant,
-                                                        crit_order=crit_order, reject_ratio=reject_ratio)
+    old = None
+    if n_iter > 1:  # rows of the active particles at t0, restored before every re-correction
+        old = dict(t=s.t[idx].copy(), dt=s.dt[idx].copy(), x=s.x[idx].copy(), v=s.v[idx].copy(), pot=s.pot[idx].copy(),
+                   D=[d[idx].copy() for d in s.D])
+    for it in range(n_iter):
+        xp, vp, ap, jp = O.predict(t_next, p, s.t, s.x, s.v, s.D)  # corrected rows have t = t_next: tau = 0
+        acc, jerk, snap, crk, pot = O.force(s.m, xp, vp, ap, jp, idx, p, eps2)
+        if it > 0:
+            s.t[idx], s.dt[idx], s.x[idx], s.v[idx], s.pot[idx] = old["t"], old["dt"], old["x"], old["v"], old["pot"]
+            for k in range(8):
+                s.D[k][idx] = old["D"][k]
+        nrej = O.correct(idx, p, t_next, eta, dt_min, dt_max, s.t, s.dt, s.x, s.v, s.D, s.pot, acc, jerk, snap, crk,
+                         pot, variant=variant, crit_order=crit_order,
+                         reject_ratio=reject_ratio if it == n_iter - 1 else 0)
+    s.rejected = getattr(s, "rejected", 0) + nrej
     return t_next, idx
 
 
-def integrate(s, t_end, eps2, eta, dt_min, dt_max, variant=0, max_blocks=10**9, crit_order=0, reject_ratio=0):
+def integrate(s, t_end, eps2, eta, dt_min, dt_max, variant=0, max_blocks=10**9, crit_order=0, reject_ratio=0, n_iter=1):
     nb = 0
     pairs = 0
     while nb < max_blocks:
         if float(np.min(s.t + s.dt)) > t_end:
             break
-        _, idx = block_step(s, eps2, eta, dt_min, dt_max, variant, crit_order, reject_ratio)
+        _, idx = block_step(s, eps2, eta, dt_min, dt_max, variant, crit_order, reject_ratio, n_iter)
         nb += 1
-        pairs += int(idx.shape[0]) * s.n
+        pairs += int(idx.shape[0]) * s.n * n_iter
     return nb, pairs
 
 

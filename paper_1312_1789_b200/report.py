@@ -220,13 +220,15 @@ def latency(args):
         # else waits on 2^-4, so every block until t = 2^-4 is a subset of those particles (their steps grow back to the
         # criterion's value on the way).  One call per driver over exactly the same blocks.
         r0 = np.argsort(np.linalg.norm(c["x"], axis=1))[: args.synthetic]
-        for driver in ("host", "device", "device_nograph"):
+        for driver in ("host", "device", "device_nograph", "device_fused"):
             g = mk()
             g.bootstrap()
             g.dt.fill_(2.0**-4)
             g.dt[torch.from_numpy(r0).cuda()] = 2.0**-16
             if driver == "device_nograph":
                 g.ctx.set_option("use_graph", 0)
+            if driver == "device_fused":
+                g.ctx.set_option("use_fused", 1)
             t_stop = 2.0**-4 - 2.0**-17
             g.run(t_stop, max_blocks=args.skip)
             torch.cuda.synchronize()

@@ -27,6 +27,7 @@ class Integrator:
         self.ctx = ctx if ctx is not None else nbody.Context(n, device)
         self.ctx.set_option("dt_criterion_order", int(dt_criterion_order or 0))
         self.ctx.set_option("step_reject_ratio", int(step_reject_ratio))  # R14: 0 = the textbook scheme
+        self.step_reject_ratio = int(step_reject_ratio)
         self.rejected = 0
         self.dt_criterion_order = int(dt_criterion_order) if dt_criterion_order else (4 if order >= 6 else order)
         up = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.dev)
@@ -64,39 +65,45 @@ class Integrator:
         else:
             c.initial_dt(n, self.D[0], self.D[1], self.eta_s, self.dt_min, self.dt_max, self.dt)
 
-    def block_step(self):
+    def block_step(self, n_iter=1):
+        """One host-driven block step.  n_iter > 1 = P(EC)^n (oracle/integrate.block_step): after the
+        corrector the active particles' corrected state stands in for their prediction (the predictor gives exactly
+        that at tau = 0), the force on them is evaluated again, their rows are put back to t0 (nbody_pack_rows /
+        nbody_unpack_rows) and corrected again with the new force.  Same kernels, C-ABI calls only."""
         c, n, p = self.ctx, self.n, self.order
+        snap, crk = (self.snap if p >= 6 else None), (self.crk if p >= 8 else None)
         t_next, n_act = c.next_block(n, self.t, self.dt, self.active)
-        c.predict(n, t_next, p, self.t, self.m, self.x, self.v, self.D)
-        c.force(self.active, n_act, p, self.eps2, self.acc, self.jerk, self.snap if p >= 6 else None,
-                self.crk if p >= 8 else None, self.fpot)
-        c.correct(self.active, n_act, p, t_next, self.eta, self.dt_min, self.dt_max, self.t, self.dt, self.x, self.v,
-                  self.D, self.pot, self.acc, self.jerk, self.snap if p >= 6 else None,
-                  self.crk if p >= 8 else None, self.fpot)
+        if n_iter > 1:
+            if getattr(self, "_rows", None) is None:
+                self._rows = torch.zeros(n, 9 + 3 * 8, dtype=torch.float64, device=self.dev)
+            c.pack_rows(self.active, n_act, 8, self.t, self.dt, self.pot, self.x, self.v, self.D, self._rows)
+        for it in range(n_iter):
+            c.predict(n, t_next, p, self.t, self.m, self.x, self.v, self.D)
+            c.force(self.active, n_act, p, self.eps2, self.acc, self.jerk, snap, crk, self.fpot)
+            if it > 0:
+                c.unpack_rows(self.active, n_act, 8, self.t, self.dt, self.pot, self.x, self.v, self.D, self._rows)
+            if it < n_iter - 1 and self.step_reject_ratio:
+                c.set_option("step_reject_ratio", 0)  # R14 applies to the last evaluation only
+            c.correct(self.active, n_act, p, t_next, self.eta, self.dt_min, self.dt_max, self.t, self.dt, self.x, self.v,
+                      self.D, self.pot, self.acc, self.jerk, snap, crk, self.fpot)
+            if it < n_iter - 1 and self.step_reject_ratio:
+                c.set_option("step_reject_ratio", self.step_reject_ratio)
         self.time = t_next
         self.blocks += 1
-        self.pairs += n_act * n
+        self.pairs += n_act * n * n_iter
         return t_next, n_act
 
-    def integrate(self, t_end, max_blocks=10**9):
-        """Advance until the next block time would exceed t_end."""
+    def integrate(self, t_end, max_blocks=10**9, n_iter=1):
+        """Host-driven integration: advance until the next block time would exceed t_end.  Returns the block-size
+        histogram {floor(log2 n_act): count}."""
         hist = {}
         while self.blocks < max_blocks:
-            # peek: the selection itself tells us t_next; stop when it passes t_end
+            # peek: the selection itself tells us t_next; stop when it passes t_end (block_step selects again: the
+            # selection is idempotent)
             t_next, n_act = self.ctx.next_block(self.n, self.t, self.dt, self.active)
             if t_next > t_end:
                 break
-            p = self.order
-            c = self.ctx
-            c.predict(self.n, t_next, p, self.t, self.m, self.x, self.v, self.D)
-            c.force(self.active, n_act, p, self.eps2, self.acc, self.jerk, self.snap if p >= 6 else None,
-                    self.crk if p >= 8 else None, self.fpot)
-            c.correct(self.active, n_act, p, t_next, self.eta, self.dt_min, self.dt_max, self.t, self.dt, self.x,
-                      self.v, self.D, self.pot, self.acc, self.jerk, self.snap if p >= 6 else None,
-                      self.crk if p >= 8 else None, self.fpot)
-            self.time = t_next
-            self.blocks += 1
-            self.pairs += n_act * self.n
+            self.block_step(n_iter)
             b = int(n_act).bit_length() - 1
             hist[b] = hist.get(b, 0) + 1
         return hist

@@ -316,3 +316,52 @@ def test_flyby_step_rejection_gpu(nb, order):
     assert a[1] == b[1] and a[2] == b[2] and np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
     ang = np.degrees(np.arctan2(a[4][0][1], a[4][0][0]))
     assert abs(abs(ang) - 90.0) < 2.5
+
+
+@pytest.mark.parametrize("order", [4, 6, 8])
+def test_pec2_block_step_vs_oracle(nb, order):
+    """N4 P(EC)^2 on the CUDA path against the oracle's P(EC)^2, lock-step from identical states: same membership, same
+    times, corrected rows within the derived corrector bound; the step uses only C-ABI calls (predict, force, correct,
+    pack_rows, unpack_rows)."""
+    import torch
+    from oracle import integrate as OI
+    from paper_1312_1789_b200.scheduler import Integrator
+    c = W.cluster(5, 513)
+    eps2 = 1e-6
+    DTMAX = 2.0**-6
+    so = OI.bootstrap(c["m"], c["x"], c["v"], order, eps2, dt_max=DTMAX)
+    g = Integrator(c["m"], c["x"], c["v"], order, eps2, dt_max=DTMAX)
+    for b in range(25):
+        for k in range(8):
+            g.D[k].copy_(U.dev(so.D[k]))
+        for dst, src in ((g.t, so.t), (g.dt, so.dt), (g.x, so.x), (g.v, so.v), (g.pot, so.pot)):
+            dst.copy_(U.dev(src))
+        h_old = so.dt.copy()
+        tn_o, idx_o = OI.block_step(so, eps2, 0.1, 2.0**-30, DTMAX, n_iter=2)
+        tn_g, na_g = g.block_step(n_iter=2)
+        torch.cuda.synchronize()
+        assert tn_g == tn_o and na_g == idx_o.shape[0]
+        assert np.array_equal(g.active[:na_g].cpu().numpy(), idx_o)
+        assert np.array_equal(g.t.cpu().numpy(), so.t)
+        # two evaluations: the second force sees the first corrector's (slightly different) x1, v1, so allow twice the bound
+        bx, bv = U.corrector_bounds(order, h_old[idx_o], [d[idx_o] for d in so.D])
+        ex = np.linalg.norm(g.x.cpu().numpy()[idx_o] - so.x[idx_o], axis=1)
+        ev = np.linalg.norm(g.v.cpu().numpy()[idx_o] - so.v[idx_o], axis=1)
+        assert np.all(ex <= 2 * bx + 1e-15) and np.all(ev <= 2 * bv + 1e-15)
+    # energy behaviour on the GPU: Kepler ellipse, shared step, P(EC)^1 drifts, P(EC)^2 does not
+    m = np.array([0.5, 0.5])
+    x = np.array([[0.25, 0, 0], [-0.25, 0, 0]])
+    v = np.array([[0, np.sqrt(3) / 2, 0], [0, -np.sqrt(3) / 2, 0]])
+
+    def en(g):
+        xx, vv = g.x.cpu().numpy(), g.v.cpu().numpy()
+        return 0.5 * np.sum(m * np.sum(vv * vv, axis=1)) - 0.25 / np.linalg.norm(xx[0] - xx[1])
+
+    err = {}
+    for n_iter in (1, 2):
+        g = Integrator(m, x, v, 4, 0.0, dt_min=2.0**-5, dt_max=2.0**-5)
+        g.bootstrap(fixed_dt=2.0**-5)
+        e0 = en(g)
+        g.integrate(64.0, n_iter=n_iter)
+        err[n_iter] = abs((en(g) - e0) / e0)
+    assert err[2] < 0.5 * err[1], err

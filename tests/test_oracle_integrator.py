@@ -596,3 +596,28 @@ def test_step_rejection_rule_details():
                 assert np.array_equal(s["x"][i], ref["x"][i]) and np.array_equal(s["D"][2][i], ref["D"][2][i])
             else:
                 assert s["t"][i] == h and s["pot"][i] == -1.0
+
+
+# ------------------------------------------------------------------------------------------- N4: P(EC)^n
+@pytest.mark.parametrize("order", [4, 6])
+def test_pec_n_iteration_removes_secular_energy_drift(order):
+    """P(EC)^n (oracle/integrate.block_step n_iter): with a shared constant step the iterated corrector converges to the
+    implicit, time-symmetric Hermite scheme, whose energy error on a Kepler ellipse (e = 0.5) stays bounded, while the
+    single-pass P(EC)^1 drifts linearly with time -- the textbook property, no formula of ours involved."""
+    m = np.array([0.5, 0.5])
+    x = np.array([[0.25, 0, 0], [-0.25, 0, 0]])
+    v = np.array([[0, math.sqrt(3) / 2, 0], [0, -math.sqrt(3) / 2, 0]])
+    dt = 2.0**-5
+    drift = {}
+    for n_iter in (1, 2, 3):
+        s = OI.bootstrap(m, x, v, order, 0.0, fixed_dt=dt)
+        e0 = _energy2(s.m, s.x, s.v)
+        errs = []
+        for T in (16.0, 64.0):
+            OI.integrate(s, T, 0.0, 1e-30, dt, dt, crit_order=order, n_iter=n_iter)
+            errs.append(abs((_energy2(s.m, s.x, s.v) - e0) / e0))
+        drift[n_iter] = errs
+    assert drift[1][1] / drift[1][0] > 10.0      # secular growth (4 x the time: ~ 50 x here, the phase error feeds back)
+    assert drift[2][1] / drift[2][0] < 1.5 and drift[3][1] / drift[3][0] < 1.5   # bounded
+    assert abs(drift[3][1] - drift[2][1]) < 0.05 * drift[2][1]                 # n = 2 is already converged to a few %
+    assert drift[2][1] < drift[1][1]
