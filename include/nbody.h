@@ -85,8 +85,8 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 ascending (hence unique) and in [0, n), nbody_correct additionally that t[i] + dt[i] == t_now for
  *                 every active i; a violation returns NBODY_EINVAL before any arithmetic.  Synchronises `stream`.
  *   "use_graph"   1 = nbody_run_blocks replays its launches as CUDA graphs [default]; 0 = plain launches
- *   "use_fused"   N1, fused small-block step.  0 [default] = every block of a run goes through the general step (five
- *                 launches: selection, predictor, force, reduce, corrector).  1 = blocks that fit one i-tile (n_act <=
+ *   "use_fused"   N1, fused small-block step.  0 [default] = every block of a run goes through the general step (four
+ *                 launches: selection, predictor, force, reduce + corrector).  1 = blocks that fit one i-tile (n_act <=
  *                 1024) go through TWO launches: selection + a persistent kernel whose CTAs predict their j-tiles on the
  *                 fly from the raw fp64 state (TMA-staged; the bit-exact predictor arithmetic) before the pair loop, and
  *                 whose last CTA sums the j-split partials and runs the corrector; a larger block ends such a batch and is
@@ -229,7 +229,7 @@ int nbody_step_host(nbody_ctx *ctx, int64_t n, int order, double eps2, double et
  * nbody_run_blocks -- N2, the device-driven block step ("individual hierarchically block time-steps";
  * PAPER.md:65 eq. (1): the latency term).  Runs whole block steps a-1 .. a-4 (selection, predict, force, correct)
  * back to back WITHOUT the host learning n_act: the selection kernel leaves t_next, n_act and the force geometry in a
- * device control block, the other kernels read them there (persistent grids of fixed size), and the five launches of
+ * device control block, the other kernels read them there (persistent grids of fixed size), and the four launches of
  * one block step are replayed as ONE CUDA graph.  The host looks at the control block only every 4 .. 64 block
  * steps.  A block is executed iff t_next <= t_end, n_act <= max_n_act and fewer than max_blocks blocks have run; the
  * first block that is not executed ends the run (the state is then exactly the state before that block).

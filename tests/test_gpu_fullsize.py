@@ -125,3 +125,34 @@ def test_full_size_physically_consistent_derivatives(config, order):
         json.dump(line, f, indent=1)
     U.check_force(got, ref, order, "cfg%d full size, bootstrap derivatives" % config)
     g.ctx.close()
+
+
+def test_double_single_mode_order4_full_size():
+    """diff_mode 1 (double-single positions, |dd|/|d| <= 1.2e-7 instead of 6e-8; R10 note) at config 2's full size,
+    4th order, ALL 65 536 particles against the oracle, with the conditioning report; the literal mode beside it.  The
+    option stays off by default (BASELINE.json words the contract as "differences formed in fp64"): this is the evidence
+    for what it would cost in accuracy."""
+    import torch
+    from paper_1312_1789_b200 import nbody
+    from oracle import oracle as O
+    c = W.cluster(2)
+    n, order, eps2 = c["n"], 4, c["eps2"]
+    idx = np.arange(n, dtype=np.int32)
+    D = [np.zeros((n, 3)), np.zeros((n, 3))]
+    t = np.zeros(n)
+    ref = O.force(c["m"], c["x"], c["v"], None, None, idx, order, eps2)
+    absn = O.force_abs(c["m"], c["x"], c["v"], None, None, idx, order, eps2)
+    radius = np.linalg.norm(c["x"], axis=1)
+    out = {}
+    for mode in (0, 1):
+        ctx = nbody.Context(n)
+        ctx.set_option("diff_mode", mode)
+        got = U.gpu_force(ctx, n, order, eps2, 0.0, t, c["m"], c["x"], c["v"], D, idx)
+        out[mode] = U.conditioning_report(got, ref, absn, radius, order)
+        U.check_force(got, ref, order, "cfg2 full size diff_mode %d" % mode)
+        ctx.close()
+    line = dict(test="double_single_order4_full_size", config=2, n=n, order=order, literal=out[0], double_single=out[1])
+    print(json.dumps(line))
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", "parity_fullsize_cfg2_diffmodes.json"), "w") as f:
+        json.dump(line, f, indent=1)
