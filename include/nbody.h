@@ -92,6 +92,15 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 whose last CTA sums the j-split partials and runs the corrector; a larger block ends such a batch and is
  *                 taken by the general step.  Bit-identical results either way.  Off by default because it is not yet
  *                 faster (profiles/r02_latency.md: one 53 KB raw stage in flight per SM is latency-bound).
+ *   "corrector_order_limit" R15, corrector order limiter (a reading added by this build; the paper is silent): 0 = off
+ *                 [default]; 1 = the corrector's velocity line is a sum of K = p/2 quadrature terms T_1 = h/2 (a0+a1),
+ *                 T_2 = w2 (j0-j1), T_3 = w3 (s0+s1), T_4 = w4 (c0-c1); M = the number of leading terms whose norms do not
+ *                 increase; a particle with M < K gets its x1, v1 from the corrector of order 2M (M = 1: trapezoid); if
+ *                 already the first end-point correction h/2 (a1 - a0) exceeds h a0 (an acceleration spike on the end
+ *                 point), M = 0: x1, v1 are the particle's own fp64 Taylor prediction and the end point is not used.  On
+ *                 smooth steps the terms fall off geometrically and nothing changes (bit-identical results); when an
+ *                 encounter sits on an end point they grow, and the higher ones are dropped instead of summed.  Stored
+ *                 derivatives, criterion and new dt are unchanged.  Bit-exact against the oracle's limit_order.
  *   "step_reject_ratio" R14, a-posteriori step rejection (a reading added by this build; the paper is silent):
  *                 0 = off [default], the textbook scheme.  R = 2^r in [2, 2^20]: if the criterion evaluated at the END of
  *                 a particle's step asks for dt_new <= h/R and h/R >= dt_min, nbody_correct does not take the step: x, v,
@@ -190,8 +199,9 @@ int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double 
 int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
                      int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);
 
-/* Steps refused by the "step_reject_ratio" rule since the counter was last reset (nbody_run_blocks resets it at the
- * start of every run); reset != 0 clears it.  *count_host is a HOST pointer; synchronises `stream`. */
+/* count_host[0] = steps refused by the "step_reject_ratio" rule, count_host[1] = steps taken with a lower-order corrector
+ * ("corrector_order_limit"), since the counters were last reset (nbody_run_blocks resets them at the start of every run);
+ * reset != 0 clears them.  count_host is a HOST array of 2; synchronises `stream`. */
 int nbody_rejected_steps(nbody_ctx *ctx, int reset, int64_t *count_host, void *stream);
 
 /* Test hook: export the packed j-store of the last predict (n particles) into plain arrays.  xp fp64 [n][3];
@@ -252,6 +262,7 @@ typedef struct nbody_run_result {
     int32_t stop_reason;
     int32_t reserved;
     int64_t rejected;       /* steps refused by the "step_reject_ratio" rule during this run */
+    int64_t limited;        /* steps taken with a lower-order corrector ("corrector_order_limit") during this run */
     int64_t hist_log2[40];
 } nbody_run_result;
 

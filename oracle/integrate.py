@@ -45,7 +45,7 @@ def bootstrap(m, x, v, order, eps2, eta_s=0.01, dt_min=2.0**-30, dt_max=2.0**-4,
     return s
 
 
-def block_step(s, eps2, eta, dt_min, dt_max, variant=0, crit_order=0, reject_ratio=0, n_iter=1):
+def block_step(s, eps2, eta, dt_min, dt_max, variant=0, crit_order=0, reject_ratio=0, n_iter=1, limit_order=0):
     """One block step (a-1 .. a-4).  Returns (t_next, active_idx).  With reject_ratio (c-9b) a rejected particle stays at
     its old time with a shorter step, so the next block time can lie before this one; s.rejected counts them.
 
@@ -69,18 +69,20 @@ def block_step(s, eps2, eta, dt_min, dt_max, variant=0, crit_order=0, reject_rat
                 s.D[k][idx] = old["D"][k]
         nrej = O.correct(idx, p, t_next, eta, dt_min, dt_max, s.t, s.dt, s.x, s.v, s.D, s.pot, acc, jerk, snap, crk,
                          pot, variant=variant, crit_order=crit_order,
-                         reject_ratio=reject_ratio if it == n_iter - 1 else 0)
+                         reject_ratio=reject_ratio if it == n_iter - 1 else 0, limit_order=limit_order,
+                         counters=s.__dict__.setdefault("counters", {}))
     s.rejected = getattr(s, "rejected", 0) + nrej
     return t_next, idx
 
 
-def integrate(s, t_end, eps2, eta, dt_min, dt_max, variant=0, max_blocks=10**9, crit_order=0, reject_ratio=0, n_iter=1):
+def integrate(s, t_end, eps2, eta, dt_min, dt_max, variant=0, max_blocks=10**9, crit_order=0, reject_ratio=0, n_iter=1,
+              limit_order=0):
     nb = 0
     pairs = 0
     while nb < max_blocks:
         if float(np.min(s.t + s.dt)) > t_end:
             break
-        _, idx = block_step(s, eps2, eta, dt_min, dt_max, variant, crit_order, reject_ratio, n_iter)
+        _, idx = block_step(s, eps2, eta, dt_min, dt_max, variant, crit_order, reject_ratio, n_iter, limit_order)
         nb += 1
         pairs += int(idx.shape[0]) * s.n * n_iter
     return nb, pairs

@@ -326,6 +326,30 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
     }
 }
 
+/* c-6 restated for one component at a chosen order m2 = 2, 4, 6, 8 (m2 = 2 is the trapezoid rule), in the operation
+ * order of oracle_correct's own lines; used by the order limiter c-6b. */
+static void corrector_xv(int m2, double h, double x0, double v0, double a0, double a1, double j0, double j1,
+                         double s0, double s1, double c0, double c1, double *x1, double *v1)
+{
+    const double h2 = h * h, h3 = h2 * h, h4 = h3 * h;
+    double v, x;
+    if (m2 == 2) {
+        v = v0 + (h / 2.0) * (a0 + a1);
+        x = x0 + (h / 2.0) * (v0 + v);
+    } else if (m2 == 4) {
+        v = v0 + ((h / 2.0) * (a0 + a1) + (h2 / 12.0) * (j0 - j1));
+        x = x0 + ((h / 2.0) * (v0 + v) + (h2 / 12.0) * (a0 - a1));
+    } else if (m2 == 6) {
+        v = v0 + ((h / 2.0) * (a0 + a1) + ((h2 / 10.0) * (j0 - j1) + (h3 / 120.0) * (s0 + s1)));
+        x = x0 + ((h / 2.0) * (v0 + v) + ((h2 / 10.0) * (a0 - a1) + (h3 / 120.0) * (j0 + j1)));
+    } else {
+        v = v0 + ((h / 2.0) * (a0 + a1) + (((3.0 * h2) / 28.0) * (j0 - j1) + ((h3 / 84.0) * (s0 + s1) + (h4 / 1680.0) * (c0 - c1))));
+        x = x0 + ((h / 2.0) * (v0 + v) + (((3.0 * h2) / 28.0) * (a0 - a1) + ((h3 / 84.0) * (j0 + j1) + (h4 / 1680.0) * (s0 - s1))));
+    }
+    *x1 = x;
+    *v1 = v;
+}
+
 /* ------------------------------------------------------------------------ *
  * c-6 + c-7 + c-8 + c-9  Corrector and new time step for the active particles.
  * h = dt_i ; 0 = stored values at t0 = t_i ; 1 = force-call values at t1 = t_now.
@@ -359,6 +383,17 @@ void oracle_initial_dt(int64_t n, const double *acc, const double *jerk,
  * block time: the scheduler (c-11, min over t + dt) picks it next and the other particles are predicted back to
  * that time with their own polynomials.  *n_rejected (may be NULL) is incremented per rejection.
  *
+ * c-6b (R15, a reading added in round 2; the paper is silent): corrector order limiter, `limit_order` != 0.
+ * The velocity line of c-6 is a sum of K = p/2 quadrature terms T_1 = h/2 (a0+a1), T_2 = w2 (j0-j1), T_3 = w3 (s0+s1),
+ * T_4 = w4 (c0-c1) (w_k = the order-p coefficients above).  On a smooth step their norms fall off like (h/tau)^k; when
+ * an encounter sits on an end point they GROW (the end-point derivatives m v^k / r^(k+2) times h^(k+1)), and summing
+ * them is summing a divergent series.  Rule: M = the number of leading terms whose norms are non-increasing
+ * (|T_2| <= |T_1|, |T_3| <= |T_2|, ...; 1 <= M <= K); if M < K, x1 and v1 of this particle are taken from the
+ * corrector of order 2M instead (M = 1: trapezoid).  One level below: if already the first end-point correction
+ * U_1 = h/2 (a1 - a0) is larger than U_0 = h a0 (the end-point acceleration is a spike: |a1 - a0| > 2 |a0|), M = 0 and
+ * x1, v1 are the particle's own Taylor prediction (c-5 in fp64): the end point is not used at all.  Everything else of
+ * the step -- stored derivatives, criterion, new dt -- is unchanged.  *n_limited (may be NULL) counts the limited steps.
+ *
  * State arrays (in/out, [n][3] unless noted): t[n], dt[n], x, v, D[k] = a^(k)
  * for k = 0..p-1, pot_state[n].  Force arrays in active-list order [n_act][3].
  * ------------------------------------------------------------------------ */
@@ -368,7 +403,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
                     double *pot_state,
                     const double *acc, const double *jerk, const double *snap,
                     const double *crackle, const double *pot, int variant, int crit_order,
-                    int reject_ratio, int64_t *n_rejected)
+                    int reject_ratio, int64_t *n_rejected, int limit_order, int64_t *n_limited)
 {
     const int p = order;
     /* c-8b (R8b): the criterion may be evaluated on the lowest pc <= p derivatives only.
@@ -377,8 +412,8 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
     const int pc = (crit_order == 4 || crit_order == 6 || crit_order == 8)
                        ? (crit_order < p ? crit_order : p)
                        : (p >= 6 ? 4 : p);
-    int64_t rejected = 0;
-#pragma omp parallel for schedule(static) reduction(+ : rejected)
+    int64_t rejected = 0, limited = 0;
+#pragma omp parallel for schedule(static) reduction(+ : rejected, limited)
     for (int64_t ia = 0; ia < n_act; ++ia) {
         const int64_t i = active_idx[ia];
         const double h = dt[i];
@@ -435,6 +470,49 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
             xnew[c] = x1;
             vnew[c] = v1;
         }
+        if (limit_order && variant == 0) { /* c-6b */
+            const int K = p / 2;
+            const double w[4] = {h / 2.0, p == 4 ? h2 / 12.0 : p == 6 ? h2 / 10.0 : (3.0 * h2) / 28.0,
+                                 p == 6 ? h3 / 120.0 : h3 / 84.0, h4 / 1680.0};
+            double T[4][3];
+            for (int c = 0; c < 3; ++c) {
+                const int64_t q = 3 * i + c, qa = 3 * ia + c;
+                T[0][c] = w[0] * (D[0][q] + acc[qa]);
+                T[1][c] = w[1] * (D[1][q] - jerk[qa]);
+                T[2][c] = K >= 3 ? w[2] * (D[2][q] + snap[qa]) : 0.0;
+                T[3][c] = K >= 4 ? w[3] * (D[3][q] - crackle[qa]) : 0.0;
+            }
+            /* level 0: the first end-point correction U_1 = h/2 (a1 - a0) against U_0 = h a0 */
+            double U0[3], U1[3];
+            for (int c = 0; c < 3; ++c) {
+                U0[c] = h * D[0][3 * i + c];
+                U1[c] = w[0] * (acc[3 * ia + c] - D[0][3 * i + c]);
+            }
+            int M = nrm3(U1) <= nrm3(U0) ? 1 : 0;
+            while (M >= 1 && M < K && nrm3(T[M]) <= nrm3(T[M - 1])) ++M;
+            if (M == 0) { /* the end point is not to be trusted at all: the particle's own Taylor prediction (c-5, fp64) */
+                const int nd = p - 2;
+                double ck[9];
+                for (int k = 1; k <= 8; ++k) ck[k] = h / (double)k;
+                for (int c = 0; c < 3; ++c) {
+                    const int64_t q = 3 * i + c;
+                    double sx = D[nd - 1][q], sv = D[nd - 1][q];
+                    for (int k = nd - 1; k >= 1; --k) sx = D[k - 1][q] + ck[k + 2] * sx;
+                    for (int k = nd - 1; k >= 1; --k) sv = D[k - 1][q] + ck[k + 1] * sv;
+                    xnew[c] = x[q] + h * (v[q] + ck[2] * sx);
+                    vnew[c] = v[q] + h * sv;
+                }
+                limited += 1;
+            } else if (M < K) {
+                for (int c = 0; c < 3; ++c) {
+                    const int64_t q = 3 * i + c, qa = 3 * ia + c;
+                    corrector_xv(2 * M, h, x[q], v[q], D[0][q], acc[qa], D[1][q], jerk[qa],
+                                 K >= 3 ? D[2][q] : 0.0, K >= 3 ? snap[qa] : 0.0,
+                                 K >= 4 ? D[3][q] : 0.0, K >= 4 ? crackle[qa] : 0.0, &xnew[c], &vnew[c]);
+                }
+                limited += 1;
+            }
+        }
         const double *dp[8];
         for (int k = 0; k < p; ++k) dp[k] = dnew[k];
         if (p == 6 && pc == 4) dp[3] = cbar; /* only directly computed derivatives enter the criterion */
@@ -455,6 +533,7 @@ void oracle_correct(const int32_t *active_idx, int64_t n_act, int order,
         dt[i] = dt_new;
     }
     if (n_rejected) *n_rejected += rejected;
+    if (n_limited) *n_limited += limited;
 }
 
 /* ------------------------------------------------------------------------ *

@@ -35,7 +35,7 @@ def lib():
         L.oracle_initial_dt.restype = None
         L.oracle_correct.argtypes = [_ip, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
                                      _dp, _dp, _dp, _dp, C.POINTER(_dp), _dp, _dp, _dp, _dp, _dp, _dp, C.c_int, C.c_int,
-                                     C.c_int, C.POINTER(C.c_int64)]
+                                     C.c_int, C.POINTER(C.c_int64), C.c_int, C.POINTER(C.c_int64)]
         L.oracle_correct.restype = None
         L.oracle_next_block.argtypes = [C.c_int64, _dp, _dp, _dp, _ip]
         L.oracle_next_block.restype = C.c_int64
@@ -131,22 +131,25 @@ def initial_dt(acc, jerk, eta_s, dt_min, dt_max):
 
 
 def correct(active_idx, order, t_now, eta, dt_min, dt_max, t, dt, x, v, D, pot_state, acc, jerk, snap, crackle, pot,
-            variant=0, crit_order=0, reject_ratio=0):
+            variant=0, crit_order=0, reject_ratio=0, limit_order=0, counters=None):
     """c-6..c-9 (+ c-8b crit_order, c-9b reject_ratio), IN PLACE on t, dt, x, v, D[0..order-1], pot_state (all must be
     C-contiguous float64 arrays).  crit_order: 0 = automatic (criterion order 4 for order >= 6, else the order), the same
     meaning as the library's "dt_criterion_order" 0; 4 | 6 | 8 = min(order, value) (value = order: the order-p criterion
-    of c-8).  reject_ratio: 0 = no step rejection; R = 2^r >= 2 = c-9b.  Returns the number of rejected steps."""
+    of c-8).  reject_ratio: 0 = no step rejection; R = 2^r >= 2 = c-9b.  limit_order: 1 = c-6b corrector order limiter.
+    Returns the number of rejected steps; `counters` (a dict) gets "limited" += the number of order-limited steps."""
     idx = np.ascontiguousarray(active_idx, dtype=np.int32)
     for a in (t, dt, x, v, pot_state, *D[:order]):
         assert a.dtype == np.float64 and a.flags.c_contiguous
     acc, jerk, pot = _d(acc), _d(jerk), _d(pot)
     snap = _d(snap) if snap is not None else None
     crackle = _d(crackle) if crackle is not None else None
-    nrej = C.c_int64(0)
+    nrej, nlim = C.c_int64(0), C.c_int64(0)
     lib().oracle_correct(idx.ctypes.data_as(_ip), idx.shape[0], order, float(t_now), float(eta), float(dt_min),
                          float(dt_max), _p(t), _p(dt), _p(x), _p(v), _ptr_array(D, 8), _p(pot_state),
                          _p(acc), _p(jerk), _p(snap), _p(crackle), _p(pot), int(variant), int(crit_order),
-                         int(reject_ratio), C.byref(nrej))
+                         int(reject_ratio), C.byref(nrej), int(limit_order), C.byref(nlim))
+    if counters is not None:
+        counters["limited"] = counters.get("limited", 0) + int(nlim.value)
     return int(nrej.value)
 
 

@@ -452,6 +452,8 @@ int launch_correct(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, 
     A.ctl = ctl;
     A.reject_ratio = c->reject_ratio;
     A.n_rejected = &c->d_ctl->rejected;
+    A.limit_order = c->limit_order;
+    A.n_limited = &c->d_ctl->limited;
     long long blocks = ctl ? 2LL * c->sm_count : (n_act + 127) / 128;
     if (blocks > 16LL * c->sm_count) blocks = 16LL * c->sm_count;
     if (order == 4) k_correct<4><<<(unsigned)blocks, 128, 0, st>>>(A);
@@ -625,6 +627,11 @@ int nbody_set_option(nbody_ctx *h, const char *key, int64_t value) {
         c->validate = (int)value;
         return NBODY_OK;
     }
+    if (!strcmp(key, "corrector_order_limit")) {
+        if (value != 0 && value != 1) return NBODY_EINVAL;
+        c->limit_order = (int)value;
+        return NBODY_OK;
+    }
     if (!strcmp(key, "step_reject_ratio")) {
         if (value != 0 && (value < 2 || value > (1 << 20) || (value & (value - 1)) != 0)) return NBODY_EINVAL;
         c->reject_ratio = (int)value;
@@ -768,11 +775,12 @@ int nbody_rejected_steps(nbody_ctx *h, int reset, int64_t *count_host, void *str
     Ctx *c = &h->c;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long v = 0;
-    NB_CUDA(c, cudaMemcpyAsync(&v, &c->d_ctl->rejected, sizeof(v), cudaMemcpyDeviceToHost, st));
+    unsigned long long v[2] = {0, 0};  // rejected, limited are adjacent in the control block
+    NB_CUDA(c, cudaMemcpyAsync(v, &c->d_ctl->rejected, sizeof(v), cudaMemcpyDeviceToHost, st));
     if (reset) NB_CUDA(c, cudaMemsetAsync(&c->d_ctl->rejected, 0, sizeof(v), st));
     NB_CUDA(c, cudaStreamSynchronize(st));
-    *count_host = (int64_t)v;
+    count_host[0] = (int64_t)v[0];
+    count_host[1] = (int64_t)v[1];
     return NBODY_OK;
 }
 
@@ -868,6 +876,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         for (int k = 0; k < 8; ++k) CA.D[k] = k < order ? a_derivs[k] : nullptr;
         CA.acc = acc; CA.jerk = jerk; CA.snap = snap; CA.crk = crackle; CA.pot = pot;
         CA.ctl = c->d_ctl; CA.reject_ratio = c->reject_ratio; CA.n_rejected = &c->d_ctl->rejected;
+        CA.limit_order = c->limit_order; CA.n_limited = &c->d_ctl->limited;
     }
     auto enqueue_step = [&](cudaStream_t s) -> int {  // general step: any block size
         k_select<<<sgrid, kSelThreads, 0, s>>>(SA);
@@ -897,7 +906,8 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
                                   (unsigned long long)(uintptr_t)jerk, (unsigned long long)(uintptr_t)snap,
                                   (unsigned long long)(uintptr_t)crackle, (unsigned long long)(uintptr_t)pot,
                                   (unsigned long long)max_n_act,
-                                  (unsigned long long)c->reject_ratio << 40 | (unsigned long long)c->crit_order << 32 |
+                                  (unsigned long long)c->limit_order << 62 | (unsigned long long)c->reject_ratio << 40 |
+                                      (unsigned long long)c->crit_order << 32 |
                                       (unsigned long long)c->force_lanes << 16 | (unsigned long long)c->force_split,
                                   0, 0, 0, 0};
     memcpy(&key[2], &eps2, 8); memcpy(&key[3], &eta, 8); memcpy(&key[4], &dt_min, 8); memcpy(&key[5], &dt_max, 8);
@@ -964,6 +974,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     res->n_act_next = (int64_t)hc->n_act;
     res->stop_reason = hc->stop;
     res->rejected = (int64_t)hc->rejected;
+    res->limited = (int64_t)hc->limited;
     for (int b = 0; b < 40; ++b) res->hist_log2[b] = (int64_t)hc->hist[b];
     NB_CUDA(c, cudaEventRecord(h->ev_out, st));
     NB_CUDA(c, cudaStreamWaitEvent(user, h->ev_out, 0));

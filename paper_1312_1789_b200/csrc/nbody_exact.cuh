@@ -156,7 +156,35 @@ struct CorrArgs {
     const Ctl *ctl;  // device-driven step: n_act and t_now from the control block (else NULL)
     int reject_ratio;               // R14 (SURVEY c-9b analogue): 0 = off
     unsigned long long *n_rejected; // device counter of refused steps
+    int limit_order;                // R15 (oracle c-6b): corrector order limiter, 0 = off
+    unsigned long long *n_limited;  // device counter of order-limited steps
 };
+
+// R6 for one component at a chosen order m2 = 2, 4, 6, 8 (2 = trapezoid), in the oracle's operation order (c-6b).
+__device__ __forceinline__ void corrector_xv(int m2, double h, double x0, double v0, double a0, double a1, double j0,
+                                             double j1, double s0, double s1, double c0, double c1, double &x1, double &v1) {
+    const double h2 = M_(h, h), h3 = M_(h2, h), h4 = M_(h3, h);
+    const double hh = Q_(h, 2.0);
+    double v, x;
+    if (m2 == 2) {
+        v = P_(v0, M_(hh, P_(a0, a1)));
+        x = P_(x0, M_(hh, P_(v0, v)));
+    } else if (m2 == 4) {
+        const double w = Q_(h2, 12.0);
+        v = P_(v0, P_(M_(hh, P_(a0, a1)), M_(w, S_(j0, j1))));
+        x = P_(x0, P_(M_(hh, P_(v0, v)), M_(w, S_(a0, a1))));
+    } else if (m2 == 6) {
+        const double w2 = Q_(h2, 10.0), w3 = Q_(h3, 120.0);
+        v = P_(v0, P_(M_(hh, P_(a0, a1)), P_(M_(w2, S_(j0, j1)), M_(w3, P_(s0, s1)))));
+        x = P_(x0, P_(M_(hh, P_(v0, v)), P_(M_(w2, S_(a0, a1)), M_(w3, P_(j0, j1)))));
+    } else {
+        const double w2 = Q_(M_(3.0, h2), 28.0), w3 = Q_(h3, 84.0), w4 = Q_(h4, 1680.0);
+        v = P_(v0, P_(M_(hh, P_(a0, a1)), P_(M_(w2, S_(j0, j1)), P_(M_(w3, P_(s0, s1)), M_(w4, S_(c0, c1))))));
+        x = P_(x0, P_(M_(hh, P_(v0, v)), P_(M_(w2, S_(a0, a1)), P_(M_(w3, P_(j0, j1)), M_(w4, S_(s0, s1))))));
+    }
+    x1 = x;
+    v1 = v;
+}
 
 template <int ORDER>
 __device__ __forceinline__ void correct_one(const CorrArgs &A, long long ia, double t_now);
@@ -243,6 +271,56 @@ __device__ __forceinline__ void correct_one(const CorrArgs &A, const long long i
         dt_new = new_dt<6>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
     else
         dt_new = new_dt<ORDER>(dn, t_now, h, A.eta, A.k_min, A.k_max, A.dt_min, A.dt_max);
+    if (A.limit_order) {  // R15 (oracle c-6b): use the highest corrector order whose quadrature terms do not grow
+        constexpr int K = ORDER / 2;
+        const double w[4] = {Q_(h, 2.0), ORDER == 4 ? Q_(h2, 12.0) : ORDER == 6 ? Q_(h2, 10.0) : Q_(M_(3.0, h2), 28.0),
+                             ORDER == 6 ? Q_(h3, 120.0) : Q_(h3, 84.0), Q_(h4, 1680.0)};
+        double T[4][3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const long long q = 3 * i + c, qa = 3 * ia + c;
+            T[0][c] = M_(w[0], P_(A.D[0][q], A.acc[qa]));
+            T[1][c] = M_(w[1], S_(A.D[1][q], A.jerk[qa]));
+            T[2][c] = K >= 3 ? M_(w[2], P_(A.D[2][q], A.snap[qa])) : 0.0;
+            T[3][c] = K >= 4 ? M_(w[3], S_(A.D[3][q], A.crk[qa])) : 0.0;
+        }
+        // level 0: the first end-point correction U_1 = h/2 (a1 - a0) against U_0 = h a0
+        double U0[3], U1[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            U0[c] = M_(h, A.D[0][3 * i + c]);
+            U1[c] = M_(w[0], S_(A.acc[3 * ia + c], A.D[0][3 * i + c]));
+        }
+        int M = nrm3(U1) <= nrm3(U0) ? 1 : 0;
+        while (M >= 1 && M < K && nrm3(T[M]) <= nrm3(T[M - 1])) ++M;
+        if (M == 0) {  // the end point is not to be trusted at all: the particle's own Taylor prediction (R5, fp64)
+            constexpr int ND = ORDER - 2;
+            double ck[9];
+#pragma unroll
+            for (int k = 1; k <= 8; ++k) ck[k] = Q_(h, (double)k);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const long long q = 3 * i + c;
+                double sx = A.D[ND - 1][q], sv = A.D[ND - 1][q];
+#pragma unroll
+                for (int k = ND - 1; k >= 1; --k) sx = P_(A.D[k - 1][q], M_(ck[k + 2], sx));
+#pragma unroll
+                for (int k = ND - 1; k >= 1; --k) sv = P_(A.D[k - 1][q], M_(ck[k + 1], sv));
+                xn[c] = P_(A.x[q], M_(h, P_(A.v[q], M_(ck[2], sx))));
+                vn[c] = P_(A.v[q], M_(h, sv));
+            }
+            atomicAdd(A.n_limited, 1ull);
+        } else if (M < K) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const long long q = 3 * i + c, qa = 3 * ia + c;
+                corrector_xv(2 * M, h, A.x[q], A.v[q], A.D[0][q], A.acc[qa], A.D[1][q], A.jerk[qa],
+                             K >= 3 ? A.D[2][q] : 0.0, K >= 3 ? A.snap[qa] : 0.0, K >= 4 ? A.D[3][q] : 0.0,
+                             K >= 4 ? A.crk[qa] : 0.0, xn[c], vn[c]);
+            }
+            atomicAdd(A.n_limited, 1ull);
+        }
+    }
     if (A.reject_ratio >= 2) {  // R14: the end-point criterion says the step was >= R times too long: do not take it
         const double R = (double)A.reject_ratio;
         const double hr = Q_(h, R);

@@ -89,6 +89,7 @@ struct Ctl {
     int jl, splits;               // force geometry of the current block (force_geometry(), evaluated on the device)
     long long i_tiles;
     unsigned long long rejected;  // steps refused by the a-posteriori rule (R14) since the counter was last reset
+    unsigned long long limited;   // steps taken with a lower-order corrector (R15) since the counter was last reset
     unsigned int tickets[4];      // last-CTA tickets
     unsigned long long hist[40];  // executed blocks by floor(log2 n_act)
 };
@@ -129,6 +130,7 @@ struct Ctx {
     int validate = 0;
     int use_graph = 1;
     int use_fused = 0;     // N1: 1 = runs of blocks that fit one i-tile go through the fused step (measured no faster yet)
+    int limit_order = 0;   // R15: 1 = corrector order limiter
     int reject_ratio = 0;  // R14: 0 = off; R = 2^r >= 2: a step whose end-point criterion asks for dt <= h/R is refused
     // bookkeeping
     int last_cuda_error = 0;

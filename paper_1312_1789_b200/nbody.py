@@ -28,7 +28,7 @@ _dbl = C.c_double
 class RunResult(C.Structure):
     """nbody_run_result of include/nbody.h."""
     _fields_ = [("blocks", C.c_int64), ("pairs", C.c_int64), ("t_next", C.c_double), ("n_act_next", C.c_int64),
-                ("stop_reason", C.c_int32), ("reserved", C.c_int32), ("rejected", C.c_int64),
+                ("stop_reason", C.c_int32), ("reserved", C.c_int32), ("rejected", C.c_int64), ("limited", C.c_int64),
                 ("hist_log2", C.c_int64 * 40)]
 
 
@@ -186,13 +186,16 @@ class Context:
                                           _ptr(active_idx), _ptr(acc), _ptr(jerk), _ptr(snap), _ptr(crackle), _ptr(pot),
                                           C.byref(r), _stream(stream)), "nbody_run_blocks")
         return dict(blocks=r.blocks, pairs=r.pairs, t_next=r.t_next, n_act_next=r.n_act_next,
-                    stop_reason=r.stop_reason, rejected=r.rejected, hist_log2=list(r.hist_log2))
+                    stop_reason=r.stop_reason, rejected=r.rejected, limited=r.limited, hist_log2=list(r.hist_log2))
 
     def rejected_steps(self, reset=False, stream=None) -> int:
-        v = _i64()
-        self._check(_lib.nbody_rejected_steps(self._h, int(bool(reset)), C.byref(v), _stream(stream)),
-                    "nbody_rejected_steps")
-        return int(v.value)
+        return self.step_counters(reset, stream)[0]
+
+    def step_counters(self, reset=False, stream=None):
+        """(steps refused by R14, steps order-limited by R15) since the last reset."""
+        v = (_i64 * 2)()
+        self._check(_lib.nbody_rejected_steps(self._h, int(bool(reset)), v, _stream(stream)), "nbody_rejected_steps")
+        return int(v[0]), int(v[1])
 
     def pack_rows(self, idx, n_rows, order, t, dt, pot_state, x, v, a_derivs, rec, stream=None):
         self._check(_lib.nbody_pack_rows(self._h, _ptr(idx), int(n_rows), int(order), _ptr(t), _ptr(dt), _ptr(pot_state),

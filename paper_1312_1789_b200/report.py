@@ -135,7 +135,8 @@ def integrate(args):
     order = args.order or c["order"]
     n, eps2 = c["n"], c["eps2"]
     g = Integrator(c["m"], c["x"], c["v"], order, eps2, eta=args.eta, dt_min=2.0**-args.dt_min_log2,
-                   dt_max=2.0**-args.dt_max_log2, step_reject_ratio=args.reject_ratio)
+                   dt_max=2.0**-args.dt_max_log2, step_reject_ratio=args.reject_ratio,
+                   corrector_order_limit=args.limit_order)
     t0 = time.perf_counter()
     g.bootstrap()
     torch.cuda.synchronize()
@@ -145,12 +146,13 @@ def integrate(args):
     ev = lambda: torch.cuda.Event(enable_timing=True)
     marks, hist = [], {}
     w0 = time.perf_counter()
-    pairs, rejected = 0, 0
+    pairs, rejected, limited = 0, 0, 0
     if args.driver == "device":
         while True:
             r = g.run(args.t_end, max_blocks=1 << 16)
             pairs += r["pairs"]
             rejected += r["rejected"]
+            limited += r["limited"]
             for k, v in enumerate(r["hist_log2"]):
                 if v:
                     hist[k] = hist.get(k, 0) + v
@@ -181,7 +183,7 @@ def integrate(args):
     torch.cuda.synchronize()
     wall = time.perf_counter() - w0
     if args.driver == "host":
-        rejected = g.ctx.rejected_steps()
+        rejected, limited = g.ctx.step_counters()
     t_pred = sum(a.elapsed_time(b) for a, b, _, _ in marks) * 1e-3
     t_force = sum(b.elapsed_time(cc) for _, b, cc, _ in marks) * 1e-3
     t_corr = sum(cc.elapsed_time(d) for _, _, cc, d in marks) * 1e-3
@@ -190,7 +192,7 @@ def integrate(args):
     dts = g.dt.cpu().numpy()
     print(json.dumps({"call": "integrate", "driver": args.driver, "config": args.config, "n": n, "order": order, "eta": args.eta,
                       "dt_criterion_order": g.dt_criterion_order, "step_reject_ratio": args.reject_ratio,
-                      "rejected_steps": rejected, "dt_max_log2": -args.dt_max_log2, "t_end": args.t_end, "reached_t_end": done,
+                      "rejected_steps": rejected, "corrector_order_limit": args.limit_order, "order_limited_steps": limited, "dt_max_log2": -args.dt_max_log2, "t_end": args.t_end, "reached_t_end": done,
                       "time_reached": g.time, "blocks": g.blocks, "pairs": pairs, "wall_s": wall,
                       "bootstrap_s": t_boot,
                       "split_s": ({"predict": t_pred, "force": t_force, "correct": t_corr,
@@ -308,6 +310,7 @@ def main(argv=None):
     i.add_argument("--max-seconds", type=float, default=1500.0)
     i.add_argument("--driver", default="host", choices=["host", "device"])
     i.add_argument("--reject-ratio", type=int, default=0, help="R14 a-posteriori step rejection (0 = off)")
+    i.add_argument("--limit-order", type=int, default=0, help="R15 corrector order limiter (0 = off, 1 = on)")
     l = sub.add_parser("latency")
     l.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
     l.add_argument("--n", type=int, default=65536)

@@ -14,7 +14,7 @@ from . import nbody
 
 class Integrator:
     def __init__(self, m, x, v, order, eps2, eta=0.1, eta_s=0.01, dt_min=2.0**-30, dt_max=2.0**-4, device=0,
-                 ctx=None, dt_criterion_order=None, step_reject_ratio=0):
+                 ctx=None, dt_criterion_order=None, step_reject_ratio=0, corrector_order_limit=0):
         """dt_criterion_order: None / 0 = the library's automatic choice (pc = 4 for order >= 6, R8b: with
         fp32 pair arithmetic the order-p criterion of R8 is driven by rounding noise in the interpolated derivatives
         and collapses the steps); 4 | 6 | 8 = criterion order min(order, value) (value = order: R8)."""
@@ -28,6 +28,8 @@ class Integrator:
         self.ctx.set_option("dt_criterion_order", int(dt_criterion_order or 0))
         self.ctx.set_option("step_reject_ratio", int(step_reject_ratio))  # R14: 0 = the textbook scheme
         self.step_reject_ratio = int(step_reject_ratio)
+        self.ctx.set_option("corrector_order_limit", int(corrector_order_limit))  # R15: 0 = off
+        self.limited = 0
         self.rejected = 0
         self.dt_criterion_order = int(dt_criterion_order) if dt_criterion_order else (4 if order >= 6 else order)
         up = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.dev)
@@ -119,6 +121,7 @@ class Integrator:
         self.blocks += r["blocks"]
         self.pairs += r["pairs"]
         self.rejected += r["rejected"]
+        self.limited += r["limited"]
         if r["blocks"]:
             self.time = float(self.t.max())  # diagnostic read (the last executed block's time)
         return r

@@ -365,3 +365,34 @@ def test_pec2_block_step_vs_oracle(nb, order):
         g.integrate(64.0, n_iter=n_iter)
         err[n_iter] = abs((en(g) - e0) / e0)
     assert err[2] < 0.5 * err[1], err
+
+
+def test_corrector_order_limiter_bit_exact(nb, O):
+    """R15 (oracle c-6b) on the CUDA path: same limited particles (count), same x1, v1, bit for bit; force inputs with a
+    spike in the higher derivatives of every third particle so that all truncation orders occur."""
+    import torch
+    n = 3001
+    for order in (4, 6, 8):
+        c, D, t, dt = _state(3, n, order)
+        t_now = 2.0**-10
+        idx = W.active_list(n, 1500, W.rng_for(3, 23))
+        xp, vp, ap, jp = O.predict(t_now, order, t, c["x"], c["v"], D)
+        f = [None if a is None else a.copy() for a in O.force(c["m"], xp, vp, ap, jp, idx, order, c["eps2"])]
+        for k in range(1, order // 2):  # spikes: term k+1 of particles k, k+3, ... grows past term k
+            f[k][k::3] *= 1e9
+        f[0][0::7] *= 50.0  # acceleration spikes: level 0 (predictor-only step)
+        cnt = {}
+        ot, odt, ox, ov, oD, op = t.copy(), dt.copy(), c["x"].copy(), c["v"].copy(), [d.copy() for d in D], np.zeros(n)
+        O.correct(idx, order, t_now, 0.1, 2.0**-30, 2.0**-4, ot, odt, ox, ov, oD, op, *f, limit_order=1, counters=cnt)
+        assert 0 < cnt["limited"] < idx.shape[0]
+        ctx = nb.Context(n)
+        ctx.set_option("corrector_order_limit", 1)
+        gt, gdt, gx, gv, gD, gp = U.dev(t), U.dev(dt), U.dev(c["x"]), U.dev(c["v"]), [U.dev(d) for d in D], U.zeros(n)
+        ctx.correct(U.dev(idx), idx.shape[0], order, t_now, 0.1, 2.0**-30, 2.0**-4, gt, gdt, gx, gv, gD, gp,
+                    *[None if a is None else U.dev(a) for a in f])
+        assert ctx.step_counters() == (0, cnt["limited"])
+        for a, b in ((gt, ot), (gdt, odt), (gx, ox), (gv, ov), (gp, op)):
+            assert np.array_equal(a.cpu().numpy(), b)
+        for k in range(8):
+            assert np.array_equal(gD[k].cpu().numpy(), oD[k])
+        ctx.close()

@@ -621,3 +621,105 @@ def test_pec_n_iteration_removes_secular_energy_drift(order):
     assert drift[2][1] / drift[2][0] < 1.5 and drift[3][1] / drift[3][0] < 1.5   # bounded
     assert abs(drift[3][1] - drift[2][1]) < 0.05 * drift[2][1]                 # n = 2 is already converged to a few %
     assert drift[2][1] < drift[1][1]
+
+
+# ------------------------------------------------------------------------------------------- c-6b (R15)
+def test_corrector_order_limiter_mechanics():
+    """c-6b: M = number of leading quadrature terms with non-increasing norms; a limited step takes x1, v1 from the
+    corrector of order 2M.  Checked against the oracle's own LOWER-ORDER correctors on the same inputs (those are pinned
+    by polynomial exactness above) and against the trapezoid rule written out; smooth data are left alone."""
+    rng = np.random.default_rng(12)
+    n = 40
+    idx = np.arange(n, dtype=np.int32)
+    h = 2.0**-5
+    mk = lambda sc: np.ascontiguousarray(rng.normal(0, 1, (n, 3)) * sc)
+    for order in (6, 8):
+        K = order // 2
+        for M in range(1, K + 1):
+            # derivative scales: terms T_k ~ h^k |a^(k-1)| fall off up to term M, then jump up
+            sc = [1.0, 1.0 / h * 0.1, 1.0 / h**2 * 0.01, 1.0 / h**3 * 0.001]
+            for k in range(M, K):
+                sc[k] = 1e6 / h**k
+            D = [mk(sc[k]) if k < K else mk(1.0) for k in range(8)]
+            f = [mk(sc[k]) for k in range(4)]
+            f[0] = D[0] + 0.01 * f[0]  # a smooth acceleration: |a1 - a0| << |a0| (level 0 does not fire)
+            x0, v0 = mk(1.0), mk(1.0)
+            st = lambda: dict(t=np.zeros(n), dt=np.full(n, h), x=x0.copy(), v=v0.copy(), D=[d.copy() for d in D], pot=np.zeros(n))
+            a, b = st(), st()
+            cnt = {}
+            O.correct(idx, order, h, 0.1, 2.0**-40, 1.0, a["t"], a["dt"], a["x"], a["v"], a["D"], a["pot"], f[0], f[1], f[2],
+                      f[3] if order == 8 else None, np.zeros(n), limit_order=1, counters=cnt)
+            O.correct(idx, order, h, 0.1, 2.0**-40, 1.0, b["t"], b["dt"], b["x"], b["v"], b["D"], b["pot"], f[0], f[1], f[2],
+                      f[3] if order == 8 else None, np.zeros(n))
+            assert cnt["limited"] == (n if M < K else 0), (order, M, cnt)
+            for k in range(order):  # stored derivatives and the new step are those of the unlimited corrector
+                assert np.array_equal(a["D"][k], b["D"][k])
+            assert np.array_equal(a["dt"], b["dt"])
+            if M == K:
+                assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["v"], b["v"])
+            elif M >= 2:  # equals the order-2M corrector of the oracle on the same inputs
+                lo = st()
+                O.correct(idx, 2 * M, h, 0.1, 2.0**-40, 1.0, lo["t"], lo["dt"], lo["x"], lo["v"], lo["D"], lo["pot"], f[0], f[1],
+                          f[2] if 2 * M >= 6 else None, None, np.zeros(n))
+                assert np.array_equal(a["x"], lo["x"]) and np.array_equal(a["v"], lo["v"])
+            else:  # trapezoid
+                v1 = v0 + (h / 2.0) * (D[0] + f[0])
+                x1 = x0 + (h / 2.0) * (v0 + v1)
+                assert np.array_equal(a["v"], v1) and np.array_equal(a["x"], x1)
+
+
+def test_corrector_order_limiter_level_zero_is_the_predictor():
+    """c-6b level 0: an end-point acceleration spike (|a1 - a0| > 2 |a0|) makes the step fall back on the particle's own
+    Taylor prediction -- exactly oracle_predict's x_p, v_p at tau = h -- while the stored derivatives and the new step
+    are still those of the end-point force."""
+    rng = np.random.default_rng(13)
+    n = 16
+    idx = np.arange(n, dtype=np.int32)
+    h = 2.0**-6
+    mk = lambda: np.ascontiguousarray(rng.normal(0, 1, (n, 3)))
+    for order in (4, 6, 8):
+        D = [mk() for _ in range(8)]
+        f = [mk() for _ in range(4)]
+        f[0] = 10.0 * D[0]
+        x0, v0 = mk(), mk()
+        t, dt, x, v, pot = np.zeros(n), np.full(n, h), x0.copy(), v0.copy(), np.zeros(n)
+        Dn = [d.copy() for d in D]
+        cnt = {}
+        O.correct(idx, order, h, 0.1, 2.0**-40, 1.0, t, dt, x, v, Dn, pot, f[0], f[1], f[2] if order >= 6 else None,
+                  f[3] if order >= 8 else None, np.zeros(n), limit_order=1, counters=cnt)
+        assert cnt["limited"] == n
+        xp, vp, _, _ = O.predict(h, order, np.zeros(n), x0, v0, D)
+        assert np.array_equal(x, xp) and np.array_equal(v, vp)
+        for k in range(order // 2):
+            assert np.array_equal(Dn[k], f[k])
+        assert np.all(t == h)
+
+
+def test_corrector_order_limiter_is_inert_on_smooth_runs_and_tames_the_flyby():
+    """c-6b never fires in a benign cluster integration (bit-identical state with and without it), and on the fly-by
+    whose closest approach sits on the end point of a long step it cuts the energy error by orders of magnitude without
+    going back in time (it cannot restore the accuracy of a resolved encounter: that needs short steps BEFORE the
+    encounter, which no end-point rule can give)."""
+    c = W.cluster(5, 256)
+    runs = []
+    for lim in (0, 1):
+        s = OI.bootstrap(c["m"], c["x"], c["v"], 8, c["eps2"], dt_max=2.0**-5)
+        OI.integrate(s, 2.0**-5, c["eps2"], 0.1, 2.0**-30, 2.0**-5, limit_order=lim)
+        runs.append((s.x.copy(), s.v.copy(), s.dt.copy(), s.counters.get("limited", 0)))
+    assert runs[1][3] == 0
+    for a, b in zip(runs[0][:3], runs[1][:3]):
+        assert np.array_equal(a, b)
+    for order in (4, 6, 8):
+        h0 = 2.0**-4
+        errs = []
+        for lim in (0, 1):
+            m = np.array([5e-4, 5e-4])
+            x = np.array([[-h0 / 2, 5e-4, 0.0], [h0 / 2, -5e-4, 0.0]])
+            v = np.array([[0.5, 0.0, 0.0], [-0.5, 0.0, 0.0]])
+            s = OI.bootstrap(m, x, v, order, 0.0, fixed_dt=h0, dt_min=2.0**-40, dt_max=h0)
+            e0 = _energy2(s.m, s.x, s.v)
+            OI.integrate(s, 2 * h0, 0.0, 0.1, 2.0**-40, h0, limit_order=lim)
+            errs.append(abs((_energy2(s.m, s.x, s.v) - e0) / e0))
+            if lim:
+                assert s.counters["limited"] >= 1
+        assert errs[1] < errs[0] / 1e4 and errs[1] < 3.0, (order, errs)  # O(1) of the TWO-BODY energy: the unresolved pericentre
