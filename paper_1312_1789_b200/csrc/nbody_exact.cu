@@ -281,9 +281,11 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
         long long s_max = A.n_tiles < 4 * slots ? A.n_tiles : 4 * slots;
         if (n_act > 0 && s_max > A.rows_budget / n_act) s_max = A.rows_budget / n_act;
         unsigned long long mine = ~0ull;  // (cost << 20) | s : the minimum is the cheapest s, smallest s on ties
-        for (long long sc = 1 + tid; sc <= s_max; sc += kSelThreads) {
-            const long long waves = (g.i_tiles * sc + slots - 1) / slots;
-            const unsigned long long cost = (unsigned long long)(waves * ((A.n_tiles + sc - 1) / sc + 3));
+        // 32-bit arithmetic is exact here: i_tiles < 8 * slots and sc <= 4 * slots, n_tiles < 2^23
+        const unsigned it32 = (unsigned)g.i_tiles, sl32 = (unsigned)slots, nt32 = (unsigned)A.n_tiles;
+        for (unsigned sc = 1 + tid; sc <= (unsigned)s_max; sc += kSelThreads) {
+            const unsigned waves = (it32 * sc + sl32 - 1) / sl32;
+            const unsigned long long cost = (unsigned long long)waves * ((nt32 + sc - 1) / sc + 3);
             const unsigned long long kk = (cost << 20) | (unsigned long long)sc;
             mine = kk < mine ? kk : mine;
         }
