@@ -189,12 +189,17 @@ def run_ours(args):
         lo, hi = parallel.shard_bounds(n_act, rank, world)
         act = g.active[lo:hi]
         snap, crk = (g.snap if p >= 6 else None), (g.crk if p >= 8 else None)
+        if world > 1:
+            ctx.set_option("geometry_n_act", n_act)  # summation order of the unsharded call (bit-identical shards)
         f0.record()
         ctx.force(act, hi - lo, p, eps2, g.acc, g.jerk, snap, crk, g.fpot)
         f1.record()
+        if world > 1:
+            ctx.set_option("geometry_n_act", 0)
         ctx.correct(act, hi - lo, p, t_next, g.eta, g.dt_min, g.dt_max, g.t, g.dt, g.x, g.v, g.D, g.pot, g.acc, g.jerk,
                     snap, crk, g.fpot)
-        sent = parallel.exchange_corrected(g.active, n_act, rank, world, g.t, g.dt, g.pot, g.x, g.v, g.D, p)
+        sent = parallel.exchange_corrected(g.active, n_act, rank, world, g.t, g.dt, g.pot, g.x, g.v, g.D, p,
+                                           ctx=ctx)
         e1.record()
         if timed:
             step_ms.append((e0, e1))
