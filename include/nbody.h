@@ -40,6 +40,7 @@ extern "C" {
 #define NBODY_ESTATE  (-2) /* call order: force before predict, force order > order of the last predict       */
 #define NBODY_ECUDA   (-3) /* a CUDA runtime call or launch failed; see nbody_last_cuda_error()               */
 #define NBODY_ENOMEM  (-4) /* device or host allocation failed                                                */
+#define NBODY_ESCRATCH (-5) /* nbody_force_static: the launch needs more than NBODY_FORCE_STATIC_SCRATCH_BYTES     */
 
 typedef struct nbody_ctx nbody_ctx;
 
@@ -157,6 +158,28 @@ int nbody_predict(nbody_ctx *ctx, int64_t n, double t_now, int order,
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_force(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order, double eps2,
                 double *acc, double *jerk, double *snap, double *crackle, double *pot, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_force_static -- nbody_force (a-3 + a-3b, same arithmetic, arguments, layout and errors) for callers that may
+ * not allocate: code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  The call performs no
+ * cudaMalloc / cudaFree and calls no allocating library routine, and the fp64 partials [S][NC][n_act] of a j-split
+ * launch (NC = 3 * order / 2 + 1) go to a STATIC device array of NBODY_FORCE_STATIC_SCRATCH_BYTES inside libnbody.so
+ * instead of the ctx's scratch.  Every GPU that loads the library holds that array until the process exits.
+ *   Limit: a launch that needs S * NC * n_act * 8 bytes > NBODY_FORCE_STATIC_SCRATCH_BYTES returns NBODY_ESCRATCH and
+ *   launches nothing (outputs untouched).  S is the j-split count of the same geometry rule nbody_force uses, so the
+ *   outputs are bit-identical to nbody_force's.  Every block of n_act <= 1024 particles fits on a B200 (one i-tile,
+ *   S <= 148 SMs: 148 * 13 * 1024 * 8 = 15 761 408 bytes); larger blocks fit when S * NC * n_act <= 2 097 152
+ *   (unsplit launches, S == 1, use no scratch and always fit); "force_split" can push S beyond the limit.
+ *   Sharing: all calls on a device use the same array, and it keeps the last call's contents.  Nothing in it has to
+ *   start at zero (the call writes every entry before it reads it), so consecutive calls on ONE stream are safe; two
+ *   calls that overlap on the GPU (different streams, or different ctxs on one device) RACE -- order them yourself.
+ *   Set-up: the first call on a device resolves the array's device address (cudaGetSymbolAddress, no allocation); a
+ *   call with n_act == 0 does only that, so issue one after nbody_create to keep it out of a capture.
+ * The ctx, its j-store and nbody_predict are as for nbody_force: nbody_create allocates, so it comes before.
+ * ---------------------------------------------------------------------------------------------------------- */
+#define NBODY_FORCE_STATIC_SCRATCH_BYTES 16777216 /* 16 MiB */
+int nbody_force_static(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int order, double eps2,
+                       double *acc, double *jerk, double *snap, double *crackle, double *pot, void *stream);
 
 /* ------------------------------------------------------------------------------------------------------------
  * nbody_correct -- a-4, Hermite corrector + Aarseth-style block time step with power-of-two quantisation for the

@@ -493,6 +493,7 @@ const char *nbody_strerror(int code) {
         case NBODY_ESTATE: return "invalid call order (predict first; force order <= predict order)";
         case NBODY_ECUDA: return "CUDA runtime error (see nbody_last_cuda_error)";
         case NBODY_ENOMEM: return "out of memory";
+        case NBODY_ESCRATCH: return "nbody_force_static: S * NC * n_act * 8 bytes exceeds NBODY_FORCE_STATIC_SCRATCH_BYTES";
         default: return "unknown nbody error code";
     }
 }
@@ -691,6 +692,29 @@ int nbody_force(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int orde
         if (rc != NBODY_OK) return rc;
     }
     return launch_force(c, active_idx, n_act, order, (float)eps2, acc, jerk, snap, crackle, pot, (cudaStream_t)stream);
+}
+
+int nbody_force_static(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int order, double eps2, double *acc,
+                       double *jerk, double *snap, double *crackle, double *pot, void *stream) {
+    if (!h || (order != 4 && order != 6 && order != 8) || n_act < 0) return NBODY_EINVAL;
+    Ctx *c = &h->c;
+    if (!(eps2 >= 0.0) || isinf(eps2)) return NBODY_EINVAL;
+    if (eps2 > 0.0 && (float)eps2 < 1.17549435e-38f) return NBODY_EINVAL;  // would flush to 0 in the fp32 pair arithmetic
+    if (c->n < 0 || order > c->pred_order) return NBODY_ESTATE;
+    if (n_act > c->n) return NBODY_EINVAL;
+    DeviceGuard guard(c->device);
+    if (n_act == 0)  // set-up only: resolves the static array's device address on this device
+        return launch_force_static(c, nullptr, 0, order, (float)eps2, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (!active_idx || !acc || !jerk || !pot || (order >= 6 && !snap) || (order >= 8 && !crackle)) return NBODY_EINVAL;
+    NB_ALIGN8(acc, jerk, snap, crackle, pot);
+    if (misaligned(active_idx, 4)) return NBODY_EINVAL;
+    if (c->diff_mode == 1 && !c->ds_valid) return NBODY_ESTATE;
+    if (c->validate) {
+        const int rc = validate_active(c, active_idx, n_act, c->n, nullptr, nullptr, 0.0, (cudaStream_t)stream);
+        if (rc != NBODY_OK) return rc;
+    }
+    return launch_force_static(c, active_idx, n_act, order, (float)eps2, acc, jerk, snap, crackle, pot,
+                               (cudaStream_t)stream);
 }
 
 int nbody_correct(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int order, double t_now, double eta,

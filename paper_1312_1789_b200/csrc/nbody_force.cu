@@ -27,6 +27,8 @@
 //     (device-driven block step, nbody_run_blocks); k_finish_dyn is K_reduce + K_corr of that step in one launch.
 #include <math.h>
 
+#include <mutex>
+
 #include "nbody_exact.cuh"
 #include "nbody_internal.h"
 
@@ -1002,6 +1004,77 @@ int launch_finish_dyn(Ctx *c, int order, const CorrArgs &corr, double *acc, doub
     else if (order == 6) k_finish_dyn<6><<<grid, 256, 0, st>>>(c->d_ctl, c->partials, corr, acc, jerk, snap, crackle, pot);
     else k_finish_dyn<8><<<grid, 256, 0, st>>>(c->d_ctl, c->partials, corr, acc, jerk, snap, crackle, pot);
     NB_CUDA(c, cudaGetLastError());
+    return NBODY_OK;
+}
+
+// ---- allocation-free K_force: the j-split scratch in static device memory (include/nbody.h, nbody_force_static) ----
+// For callers that may not allocate (and that do not want the launch to touch ctx-owned scratch): the [S][NC][n_act] fp64
+// partials of a j-split launch go to this file-scope array instead of Ctx::partials.  Every GPU that loads libnbody.so
+// holds the array (NBODY_FORCE_STATIC_SCRATCH_BYTES = 16 MiB) until the process exits.  All calls on a device share it,
+// so two nbody_force_static launches that overlap on the GPU (different streams) race; launches on one stream do not.
+// Nothing in it has to start at zero: K_force writes every entry (split, component, slot < n_act) that K_reduce of the
+// same call reads, so the previous call's contents are never seen.
+static __device__ __align__(256) double g_force_static_scratch[NBODY_FORCE_STATIC_SCRATCH_BYTES / sizeof(double)];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+double *g_static_scratch_ptr[kMaxDevices] = {nullptr};  // device address of the array, per device (host code cannot
+std::mutex g_static_scratch_mutex;                      // use the symbol's name: that is a host-side stand-in)
+
+// Set-up, once per device, with that device current (the caller holds a DeviceGuard): resolve the device address.
+int static_scratch_address(Ctx *c, double **out) {
+    if (c->device < 0 || c->device >= kMaxDevices) return NBODY_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_scratch_mutex);
+    if (!g_static_scratch_ptr[c->device]) {
+        double *ptr = nullptr;
+        NB_CUDA(c, cudaGetSymbolAddress((void **)&ptr, g_force_static_scratch));
+        if (!ptr) return NBODY_ECUDA;
+        g_static_scratch_ptr[c->device] = ptr;
+    }
+    *out = g_static_scratch_ptr[c->device];
+    return NBODY_OK;
+}
+
+}  // namespace
+
+// launch_force with the split partials in the static array: same kernels, same geometry rule (so the same bits as
+// launch_force for the same options), no allocation, Ctx::partials untouched.  n_act == 0 only resolves the address.
+int launch_force_static(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, float eps2, double *acc, double *jerk,
+                        double *snap, double *crackle, double *pot, cudaStream_t st) {
+    double *scratch = nullptr;
+    const int rc = static_scratch_address(c, &scratch);
+    if (rc != NBODY_OK) return rc;
+    if (n_act == 0) return NBODY_OK;
+    const int K = order / 2, NC = 3 * K + 1;
+    ForceArgs A;
+    fill_args(c, A, active_idx, eps2, acc, jerk, snap, crackle, pot);
+    A.partials = scratch;
+    const int64_t n_geo = c->geometry_n_act ? c->geometry_n_act : n_act;
+    if (n_act > n_geo) return NBODY_EINVAL;
+    const ForceGeo g = force_geometry(n_geo, A.n_tiles, c->sm_count, c->force_lanes, c->force_split, c->partial_rows);
+    const int64_t i_tiles = (n_act + g.i_per_cta - 1) / g.i_per_cta;
+    if (g.splits > 1 &&
+        (uint64_t)g.splits * (uint64_t)NC * (uint64_t)n_act * sizeof(double) > (uint64_t)NBODY_FORCE_STATIC_SCRATCH_BYTES)
+        return NBODY_ESCRATCH;  // beyond the static array: nothing was launched
+    A.n_act = (int)n_act;
+    A.splits = g.splits;
+    const dim3 grid((unsigned)i_tiles, (unsigned)g.splits);
+    pick_fn(order, c->diff_mode, g.jl)<<<grid, kThreads, smem_for(order, c->diff_mode), st>>>(A);
+    c->launches += 1;
+    NB_CUDA(c, cudaGetLastError());
+    if (g.splits > 1) {
+        const long long tot = (long long)NC * n_act;
+        long long blocks = g.splits <= 8 ? (tot + 255) / 256 : (tot + 7) / 8;  // thread or warp per output
+        if (blocks > 8LL * c->sm_count) blocks = 8LL * c->sm_count;
+        k_reduce<<<(unsigned)blocks, 256, 0, st>>>(scratch, g.splits, NC, (int)n_act, acc, jerk, snap, crackle, pot);
+        c->launches += 1;
+        NB_CUDA(c, cudaGetLastError());
+    }
+    c->last_r = 2;
+    c->last_jl = g.jl;
+    c->last_s = g.splits;
+    c->last_ctas = i_tiles * g.splits;
     return NBODY_OK;
 }
 

@@ -184,6 +184,9 @@ int launch_force(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, fl
 // device-driven variant: n_act and the geometry are read from the control block on the device
 int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, double *acc, double *jerk, double *snap,
                      double *crackle, double *pot, cudaStream_t st);
+// allocation-free variant: split partials in the library's static device array (nbody_force_static)
+int launch_force_static(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, float eps2, double *acc, double *jerk,
+                        double *snap, double *crackle, double *pot, cudaStream_t st);
 int force_static_init(Ctx *c);
 struct CorrArgs;
 // device-driven step: K_reduce + K_corr in one launch (reads n_act, S, t_next from the control block)

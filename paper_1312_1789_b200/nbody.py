@@ -19,7 +19,8 @@ if not os.path.exists(LIB_PATH):
 
 _lib = C.CDLL(LIB_PATH)
 
-OK, EINVAL, ESTATE, ECUDA, ENOMEM = 0, -1, -2, -3, -4
+OK, EINVAL, ESTATE, ECUDA, ENOMEM, ESCRATCH = 0, -1, -2, -3, -4, -5
+FORCE_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # NBODY_FORCE_STATIC_SCRATCH_BYTES (include/nbody.h)
 
 _vp = C.c_void_p
 _i64 = C.c_int64
@@ -43,6 +44,7 @@ SIGNATURES = {
     "nbody_set_option": (C.c_int, [_vp, C.c_char_p, _i64]),
     "nbody_predict": (C.c_int, [_vp, _i64, _dbl, C.c_int, _vp, _vp, _vp, _vp, C.POINTER(_vp), _vp]),
     "nbody_force": (C.c_int, [_vp, _vp, _i64, C.c_int, _dbl, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nbody_force_static": (C.c_int, [_vp, _vp, _i64, C.c_int, _dbl, _vp, _vp, _vp, _vp, _vp, _vp]),
     "nbody_correct": (C.c_int, [_vp, _vp, _i64, C.c_int, _dbl, _dbl, _dbl, _dbl, _vp, _vp, _vp, _vp, C.POINTER(_vp),
                                 _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "nbody_initial_dt": (C.c_int, [_vp, _i64, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
@@ -152,6 +154,13 @@ class Context:
     def force(self, active_idx, n_act, order, eps2, acc, jerk, snap, crackle, pot, stream=None):
         self._check(_lib.nbody_force(self._h, _ptr(active_idx), int(n_act), int(order), float(eps2), _ptr(acc),
                                      _ptr(jerk), _ptr(snap), _ptr(crackle), _ptr(pot), _stream(stream)), "nbody_force")
+
+    def force_static(self, active_idx, n_act, order, eps2, acc, jerk, snap, crackle, pot, stream=None):
+        """nbody_force with the j-split scratch in the library's static device array (no allocation; the launch
+        must need <= FORCE_STATIC_SCRATCH_BYTES, else NBODY_ESCRATCH)."""
+        self._check(_lib.nbody_force_static(self._h, _ptr(active_idx), int(n_act), int(order), float(eps2), _ptr(acc),
+                                            _ptr(jerk), _ptr(snap), _ptr(crackle), _ptr(pot), _stream(stream)),
+                    "nbody_force_static")
 
     def correct(self, active_idx, n_act, order, t_now, eta, dt_min, dt_max, t, dt, x, v, a_derivs, pot_state,
                 acc, jerk, snap, crackle, pot, stream=None):
