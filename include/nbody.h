@@ -216,8 +216,10 @@ int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double 
 /* ------------------------------------------------------------------------------------------------------------
  * nbody_next_block -- a-1, block selection on the device (R9c = SURVEY c-11): t_next = min_i (t[i] + dt[i])
  * (exact for dyadic values); active = { i : t[i] + dt[i] == t_next } ascending.  Writes active_idx (device
- * int32, capacity n) and returns t_next and n_act through HOST pointers; this call synchronises `stream`.
- * One kernel (a persistent grid with two grid barriers: min | count | ordered write).
+ * int32, capacity n: entries [0, n_act) are the block, entries at and beyond n_act are scratch and may be
+ * overwritten) and returns t_next and n_act through HOST pointers; this call synchronises `stream`.
+ * One kernel, one pass, no grid barrier: every CTA lists the particles of its chunk due at the chunk's own minimum;
+ * the last CTA to finish takes the global minimum and concatenates the lists that belong to it, in order.
  * ---------------------------------------------------------------------------------------------------------- */
 int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
                      int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);

@@ -117,15 +117,21 @@ __global__ void k_initial_dt(long long n, const double *acc, const double *jerk,
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------
-// Block selection (a-1, R9c) in ONE kernel: min of t + dt, then order-preserving compaction of the particles due
-// at it.  A persistent grid (<= one CTA per SM, all resident) with two grid barriers: [min] | [count] | [write].
-// The last phase also leaves the block time, the block size, the force geometry (force_geometry(), evaluated by
-// 1024 threads in parallel) and the run bookkeeping in the device control block, so that the rest of the block
-// step can be launched without the host knowing n_act (nbody_run_blocks).
+// Block selection (a-1, R9c) in ONE kernel, one pass, no grid barrier.  Every CTA owns a contiguous chunk of the
+// particles: it takes the chunk's own minimum of t + dt and writes the indices of the chunk's particles due at THAT
+// time, in order, to its slice of a candidate array.  The last CTA to finish (ticket) takes the minimum over the
+// CTAs, concatenates the candidate lists of the CTAs whose minimum it is -- in CTA order, so the active list is
+// ascending -- and leaves the block time, the block size, the force geometry (force_geometry(), evaluated by 1024
+// threads in parallel) and the run bookkeeping in the device control block, so that the rest of the block step can be
+// launched without the host knowing n_act (nbody_run_blocks).  The concatenation is a copy of at most n_act indices by
+// one CTA (n_act * 8 bytes against n_act * n pair interactions of the force call that follows); every CTA also writes
+// its list to the same place of the active list, which is its final place in an all-active block: no copy then.
+// Entries of the active list at and beyond n_act are scratch.
 // ---------------------------------------------------------------------------------------------------------
 namespace {
 
 constexpr int kSelThreads = 1024;
+constexpr int kSelMaxGrid = 1024;  // CTAs of the selection kernel (<= the SM count; bounds the tail's shared arrays)
 
 // order-preserving map double -> uint64 (total order of finite values)
 __device__ __forceinline__ unsigned long long dkey(double v) {
@@ -137,30 +143,14 @@ __device__ __forceinline__ double dunkey(unsigned long long k) {
     return __longlong_as_double((long long)b);
 }
 
-__device__ __forceinline__ void grid_barrier(SelBar *bar, unsigned grid) {
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned gen = *(volatile unsigned *)&bar->gen;
-        if (atomicAdd(&bar->count, 1u) == grid - 1) {
-            bar->count = 0;
-            __threadfence();
-            atomicAdd(&bar->gen, 1u);
-        } else {
-            while (*(volatile unsigned *)&bar->gen == gen) {}
-        }
-        __threadfence();
-    }
-    __syncthreads();
-}
-
 struct SelArgs {
     long long n;
     const double *t, *dt;
     Ctl *ctl;
-    SelBar *bar;
-    int *counts;          // [grid]
-    int32_t *active_idx;  // [n]
+    unsigned long long *keys;  // [grid] minimum of each CTA's chunk
+    int *counts;               // [grid] particles of the chunk due at the CTA's own minimum
+    int32_t *cand;             // [n]    their indices, CTA b's at cand[chunk start of b ...]
+    int32_t *active_idx;       // [n]
     // force geometry inputs (force_geometry)
     int n_tiles, sm_count, force_lanes, force_split;
     long long rows_budget;
@@ -170,110 +160,173 @@ struct SelArgs {
     long long max_n_act;  // run: a block larger than this stops the run (stop = 2) for the host to handle
 };
 
-__global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
-    __shared__ unsigned long long s_key[kSelThreads / 32];
-    __shared__ int s_warp[kSelThreads / 32];
-    __shared__ long long s_base, s_all;
-    const unsigned grid = gridDim.x;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // a stopped run stays stopped (nothing after the stopping selection touches the state): replays are no-ops
-    if (A.run_mode && *(volatile int *)&A.ctl->stop) return;
-    const long long chunk = (A.n + grid - 1) / grid;
-    const long long c0 = (long long)blockIdx.x * chunk;
-    const long long c1 = c0 + chunk < A.n ? c0 + chunk : A.n;
-
-    // ---- phase 1: min of t + dt (exact for dyadic values) ----
-    unsigned long long k = ~0ull;
-    for (long long i = c0 + tid; i < c1; i += kSelThreads) {
-        const unsigned long long ki = dkey(__dadd_rn(A.t[i], A.dt[i]));
-        k = ki < k ? ki : k;
-    }
+// minimum over the CTA of a 64-bit key (every thread gets it); s_red: one slot per warp
+__device__ __forceinline__ unsigned long long cta_min_key(unsigned long long k, unsigned long long *s_red) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         const unsigned long long other = __shfl_xor_sync(0xffffffffu, k, o);
         k = other < k ? other : k;
     }
-    if (lane == 0) s_key[warp] = k;
+    if (lane == 0) s_red[warp] = k;
+    __syncthreads();
+    k = s_red[lane];  // kSelThreads / 32 == 32 slots
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, k, o);
+        k = other < k ? other : k;
+    }
+    __syncthreads();  // s_red may be reused
+    return k;
+}
+
+constexpr int kSelRows = 16;  // rows of kSelThreads consecutive particles compacted per pass (bounds the shared counts)
+
+__global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
+    extern __shared__ unsigned long long s_keys[];  // [min(rows of the chunk, kSelRows)][kSelThreads]
+    __shared__ unsigned long long s_red[kSelThreads / 32];
+    __shared__ int s_cntw[kSelRows * 32];  // due particles per (row, warp), then their exclusive offsets
+    __shared__ int s_cnt[kSelMaxGrid];
+    __shared__ long long s_off[kSelMaxGrid];
+    __shared__ long long s_all;
+    __shared__ int s_tot;
+    __shared__ bool s_last;
+    const unsigned grid = gridDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    Ctl *ctl = A.ctl;
+    // a stopped run stays stopped (nothing after the stopping selection touches the state): replays are no-ops
+    if (A.run_mode && *(volatile int *)&ctl->stop) return;
+    // run control read early (whichever CTA turns out to be the last one needs it; nobody writes it meanwhile)
+    double t_end = 0.0;
+    long long max_blocks = 0;
+    unsigned long long blocks = 0;
+    if (A.run_mode && tid == 0) {
+        t_end = ctl->t_end;
+        max_blocks = ctl->max_blocks;
+        blocks = ctl->blocks;
+    }
+    const long long chunk = (A.n + grid - 1) / grid;
+    const long long c0 = (long long)blockIdx.x * chunk;
+    const long long c1 = c0 + chunk < A.n ? c0 + chunk : A.n;
+    const long long per = (chunk + kSelThreads - 1) / kSelThreads;  // rows of this CTA's chunk
+
+    // ---- the chunk's minimum of t + dt (exact for dyadic values); row r holds particles c0 + r * 1024 + tid ----
+    unsigned long long k = ~0ull;
+#pragma unroll 4
+    for (long long r = 0; r < per; ++r) {
+        const long long i = c0 + r * kSelThreads + tid;
+        if (i < c1) {
+            const unsigned long long ki = dkey(__dadd_rn(A.t[i], A.dt[i]));
+            k = ki < k ? ki : k;
+            if (r < kSelRows) s_keys[r * kSelThreads + tid] = ki;  // the first kSelRows rows stay in shared memory
+        }
+    }
+    const unsigned long long key_cta = cta_min_key(k, s_red);
+
+    // ---- the chunk's particles due at it, in index order, to the CTA's slice of the candidate array: per row one
+    // ballot per warp, the (row, warp) counts scanned in shared memory, kSelRows rows at a time (the keys of the first
+    // kSelRows rows come from shared memory, those of later rows -- N > 2.4 M -- are recomputed from t and dt) ----
+    int base = 0;
+    for (long long r0 = 0; r0 < per; r0 += kSelRows) {
+        const int rows = per - r0 < kSelRows ? (int)(per - r0) : kSelRows;
+#pragma unroll 1
+        for (int r = 0; r < rows; ++r) {
+            const long long i = c0 + (r0 + r) * kSelThreads + tid;
+            const bool due = i < c1 && (r0 == 0 ? s_keys[r * kSelThreads + tid] : dkey(__dadd_rn(A.t[i], A.dt[i]))) == key_cta;
+            const unsigned m = __ballot_sync(0xffffffffu, due);
+            if (lane == 0) s_cntw[r * 32 + warp] = __popc(m);
+        }
+        __syncthreads();
+        if (warp == 0) {  // exclusive scan of the rows * 32 counts: lane l owns entries [l * rows, (l + 1) * rows)
+            int sum = 0;
+            for (int e = 0; e < rows; ++e) sum += s_cntw[lane * rows + e];
+            int incl = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int up = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += up;
+            }
+            int run = incl - sum;
+            for (int e = 0; e < rows; ++e) {
+                const int v = s_cntw[lane * rows + e];
+                s_cntw[lane * rows + e] = run;
+                run += v;
+            }
+            if (lane == 31) s_tot = incl;
+        }
+        __syncthreads();
+        if (s_tot) {  // uniform
+#pragma unroll 1
+            for (int r = 0; r < rows; ++r) {
+                const long long i = c0 + (r0 + r) * kSelThreads + tid;
+                const bool due = i < c1 && (r0 == 0 ? s_keys[r * kSelThreads + tid] : dkey(__dadd_rn(A.t[i], A.dt[i]))) == key_cta;
+                const unsigned m = __ballot_sync(0xffffffffu, due);
+                if (due) {  // also to the same place of the active list: a CTA whose final offset is its chunk start is done
+                    const long long q = c0 + base + s_cntw[r * 32 + warp] + __popc(m & ((1u << lane) - 1u));
+                    A.cand[q] = (int32_t)i;
+                    A.active_idx[q] = (int32_t)i;
+                }
+            }
+        }
+        base += s_tot;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        A.counts[blockIdx.x] = base;
+        A.keys[blockIdx.x] = key_cta;
+    }
+
+    // ---- ticket: the last CTA to get here finishes the selection ----
+    __threadfence();
     __syncthreads();
     if (tid == 0) {
-        for (int w = 1; w < kSelThreads / 32; ++w) k = s_key[w] < k ? s_key[w] : k;
-        atomicMin(&A.ctl->min_key, k);
+        const unsigned ticket = atomicAdd(&ctl->tickets[1], 1u);
+        s_last = ticket == grid - 1;
+        if (s_last) ctl->tickets[1] = 0;  // ready for the next selection (stream-ordered after this one)
     }
-    grid_barrier(A.bar, grid);
-    const unsigned long long key = *(volatile unsigned long long *)&A.ctl->min_key;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
 
-    // ---- phase 2: count the due particles; thread `tid` owns the contiguous run [e0, e1) of its CTA's chunk ----
-    const long long per = (chunk + kSelThreads - 1) / kSelThreads;
-    const long long e0 = c0 + (long long)tid * per < c1 ? c0 + (long long)tid * per : c1;
-    const long long e1 = e0 + per < c1 ? e0 + per : c1;
-    int cnt = 0;
-    unsigned mask = 0;  // due flags of the first 32 elements of the run (longer runs are re-read in phase 3)
-    for (long long i = e0; i < e1; ++i) {
-        const bool due = dkey(__dadd_rn(A.t[i], A.dt[i])) == key;
-        if (due) {
-            ++cnt;
-            if (i - e0 < 32) mask |= 1u << (int)(i - e0);
-        }
+    // global minimum, and the size of the block = the counts of the CTAs whose minimum it is
+    unsigned long long kb = ~0ull;
+    int cb = 0;
+    if (tid < (int)grid) {
+        kb = __ldcg(A.keys + tid);
+        cb = __ldcg(A.counts + tid);
     }
-    int incl = cnt;
+    const unsigned long long key = cta_min_key(kb, s_red);
+    if (tid < (int)grid) s_cnt[tid] = kb == key ? cb : 0;
+    __syncthreads();
+    if (warp == 0) {  // exclusive scan of s_cnt over the CTAs, 32 at a time
+        long long running = 0;
+        for (unsigned b0 = 0; b0 < grid; b0 += 32) {
+            const int v = b0 + lane < grid ? s_cnt[b0 + lane] : 0;
+            long long in = v;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int up = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += up;
-    }
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    if (tid == 0) {
-        int run = 0;
-        for (int w = 0; w < kSelThreads / 32; ++w) {
-            const int v = s_warp[w];
-            s_warp[w] = run;
-            run += v;
+            for (int o = 1; o < 32; o <<= 1) {
+                const long long up = __shfl_up_sync(0xffffffffu, in, o);
+                if (lane >= o) in += up;
+            }
+            if (b0 + lane < grid) s_off[b0 + lane] = running + in - v;
+            running += __shfl_sync(0xffffffffu, in, 31);
         }
-        A.counts[blockIdx.x] = run;
+        if (lane == 0) s_all = running;
     }
     __syncthreads();
-    const int off_in_cta = s_warp[warp] + incl - cnt;
-    grid_barrier(A.bar, grid);
+    // ordered concatenation: warp w copies the candidate lists of CTAs w, w + 32, ... (a list that already sits at its
+    // final offset -- every list of an all-active block -- is left alone)
+    for (unsigned b = warp; b < grid; b += kSelThreads / 32) {
+        const int nb = s_off[b] == (long long)b * chunk ? 0 : s_cnt[b];
+        const int32_t *src = A.cand + (long long)b * chunk;
+        int32_t *dst = A.active_idx + s_off[b];
+        for (int e = lane; e < nb; e += 32) dst[e] = __ldcg(src + e);
+    }
 
-    // ---- phase 3: global offsets, ordered write, control block ----
-    if (warp == 0) {
-        long long before = 0, all = 0;
-        for (unsigned b = lane; b < grid; b += 32) {
-            const int v = *(volatile int *)&A.counts[b];
-            all += v;
-            if (b < blockIdx.x) before += v;
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            before += __shfl_xor_sync(0xffffffffu, before, o);
-            all += __shfl_xor_sync(0xffffffffu, all, o);
-        }
-        if (lane == 0) {
-            s_base = before;
-            s_all = all;
-        }
-    }
-    __syncthreads();
-    long long pos = s_base + off_in_cta;
-    for (long long i = e0; i < e1; ++i) {
-        const bool due = (i - e0 < 32) ? ((mask >> (int)(i - e0)) & 1u) : (dkey(__dadd_rn(A.t[i], A.dt[i])) == key);
-        if (due) A.active_idx[pos++] = (int32_t)i;
-    }
-    if (blockIdx.x != 0) return;
-
-    // CTA 0: block time, size, run control, force geometry (the parallel form of force_geometry()'s search)
+    // block time, size, run control, force geometry (the parallel form of force_geometry()'s search)
     const long long n_act = s_all;
     const double t_next = dunkey(key);
-    Ctl *ctl = A.ctl;
-    int stop = 0;
-    if (A.run_mode) {
-        if (t_next > ctl->t_end) stop = 1;
-        else if (n_act > A.max_n_act) stop = 2;
-        else if ((long long)ctl->blocks >= ctl->max_blocks) stop = 3;
-    }
     ForceGeo g = force_geometry(n_act, A.n_tiles, A.sm_count, A.force_lanes, /*force_split=*/1, A.rows_budget);
-    if (A.run_mode == 2 && !stop && g.i_tiles != 1) stop = 4;  // fused small-block run: this block needs the general step
     const long long slots = A.sm_count;
     long long S = 1;
     if (A.force_split) S = A.force_split;
@@ -289,25 +342,22 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
             const unsigned long long kk = (cost << 20) | (unsigned long long)sc;
             mine = kk < mine ? kk : mine;
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long other = __shfl_xor_sync(0xffffffffu, mine, o);
-            mine = other < mine ? other : mine;
-        }
-        __syncthreads();
-        if (lane == 0) s_key[warp] = mine;
-        __syncthreads();
-        if (tid == 0) {
-            for (int w = 1; w < kSelThreads / 32; ++w) mine = s_key[w] < mine ? s_key[w] : mine;
-            if (mine != ~0ull) {
-                const long long best = (long long)(mine >> 20);
-                const long long cost1 = ((g.i_tiles + slots - 1) / slots) * ((long long)A.n_tiles + 3);
-                S = (long long)(mine & 0xfffffull);
-                if (100 * best > 97 * cost1) S = 1;
-            }
+        mine = cta_min_key(mine, s_red);
+        if (mine != ~0ull) {
+            const long long best = (long long)(mine >> 20);
+            const long long cost1 = ((g.i_tiles + slots - 1) / slots) * ((long long)A.n_tiles + 3);
+            S = (long long)(mine & 0xfffffull);
+            if (100 * best > 97 * cost1) S = 1;
         }
     }
     if (tid == 0) {
+        int stop = 0;
+        if (A.run_mode) {
+            if (t_next > t_end) stop = 1;
+            else if (n_act > A.max_n_act) stop = 2;
+            else if ((long long)blocks >= max_blocks) stop = 3;
+            else if (A.run_mode == 2 && g.i_tiles != 1) stop = 4;  // fused small-block run: this block needs the general step
+        }
         if (S > A.n_tiles) S = A.n_tiles;
         if (S > 65535) S = 65535;
         if (S < 1) S = 1;
@@ -317,13 +367,12 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select(const SelArgs A) {
         ctl->splits = (int)S;
         ctl->i_tiles = g.i_tiles;
         ctl->stop = stop;
-        ctl->min_key = ~0ull;  // every CTA has read it (second barrier): ready for the next selection
         if (A.run_mode && !stop) {
-            ctl->blocks += 1;
-            ctl->pairs += (unsigned long long)n_act * (unsigned long long)A.n;
+            ctl->blocks = blocks + 1;
+            atomicAdd(&ctl->pairs, (unsigned long long)n_act * (unsigned long long)A.n);
             int b = 0;
             while ((n_act >> (b + 1)) != 0) ++b;
-            ctl->hist[b < 39 ? b : 39] += 1;
+            atomicAdd(&ctl->hist[b < 39 ? b : 39], 1ull);
         }
     }
 }
@@ -396,16 +445,27 @@ inline bool misaligned(const void *p, size_t a) { return p && ((uintptr_t)p & (a
             if (misaligned(p__, 8)) return NBODY_EINVAL;        \
     } while (0)
 
+size_t select_smem(const Ctx *c, int64_t n);
+
 int select_grid(const Ctx *c, int64_t n) {
     int64_t g = (n + kSelThreads - 1) / kSelThreads;
     if (g > c->sm_count) g = c->sm_count;
+    if (g > kSelMaxGrid) g = kSelMaxGrid;
     return (int)(g < 1 ? 1 : g);
+}
+
+size_t select_smem(const Ctx *c, int64_t n) {  // the key cache of k_select: rows of the chunk, at most kSelRows
+    const int64_t grid = select_grid(c, n);
+    const int64_t chunk = (n + grid - 1) / grid;
+    int64_t rows = (chunk + kSelThreads - 1) / kSelThreads;
+    if (rows > kSelRows) rows = kSelRows;
+    return (size_t)rows * kSelThreads * sizeof(unsigned long long);
 }
 
 void fill_select(nbody_ctx *h, SelArgs &A, int64_t n, const double *t, const double *dt, int32_t *active_idx,
                  int run_mode, int64_t max_n_act) {
     Ctx *c = &h->c;
-    A.n = n; A.t = t; A.dt = dt; A.ctl = c->d_ctl; A.bar = h->d_bar; A.counts = c->d_counts; A.active_idx = active_idx;
+    A.n = n; A.t = t; A.dt = dt; A.ctl = c->d_ctl; A.keys = c->d_keys; A.counts = c->d_counts; A.cand = c->d_cand; A.active_idx = active_idx;
     A.n_tiles = (int)((n + kTileJ - 1) / kTileJ);
     A.sm_count = c->sm_count; A.force_lanes = c->force_lanes; A.force_split = c->force_split;
     A.rows_budget = c->partial_rows;
@@ -506,7 +566,7 @@ int64_t nbody_workspace_bytes(int64_t n_capacity) {
     if (rows * 13 * 8 > (int64_t)512 << 20) rows = ((int64_t)512 << 20) / (13 * 8);
     const int64_t n_tiles = cap_pad / kTileJ;
     if (rows > n_tiles * n_capacity) rows = n_tiles * n_capacity;
-    return (int64_t)sizeof(uint4) * kPlanes * cap_pad + rows * 13 * 8 + 4096;
+    return (int64_t)sizeof(uint4) * kPlanes * cap_pad + rows * 13 * 8 + 4 * n_capacity /* selection candidates */ + 8192;
 }
 
 int nbody_create(nbody_ctx **out, int64_t n_capacity, int device) {
@@ -540,18 +600,19 @@ int nbody_create(nbody_ctx **out, int64_t n_capacity, int device) {
         if ((e = cudaMalloc(&c->partials, c->partials_bytes)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaMalloc(&c->d_counts, sizeof(int) * (c->sm_count + 1))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaMalloc(&c->d_ctl, sizeof(Ctl))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        if ((e = cudaMalloc(&h->d_bar, sizeof(SelBar))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&c->d_keys, sizeof(unsigned long long) * (c->sm_count + 1))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
+        if ((e = cudaMalloc(&c->d_cand, sizeof(int32_t) * n_capacity)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaMalloc(&c->d_flag, sizeof(int))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaMallocHost(&c->h_ctl, sizeof(Ctl))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         memset(c->h_ctl, 0, sizeof(Ctl));
-        c->h_ctl->min_key = ~0ull;
         if ((e = cudaMemcpy(c->d_ctl, c->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
-        if ((e = cudaMemset(h->d_bar, 0, sizeof(SelBar))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaStreamCreateWithFlags(&h->run_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming)) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         rc = force_static_init(c);
         if (rc != NBODY_OK) break;
+        if ((e = cudaFuncSetAttribute((const void *)k_select, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      kSelRows * kSelThreads * (int)sizeof(unsigned long long))) != cudaSuccess) { rc = cuda_fail(c, e); break; }
         if ((e = cudaDeviceSynchronize()) != cudaSuccess) { rc = cuda_fail(c, e); break; }
     } while (0);
     if (rc != NBODY_OK) {
@@ -576,7 +637,8 @@ int nbody_destroy(nbody_ctx *h) {
     cudaFree(c->partials);
     cudaFree(c->d_counts);
     cudaFree(c->d_ctl);
-    cudaFree(h->d_bar);
+    cudaFree(c->d_keys);
+    cudaFree(c->d_cand);
     cudaFree(c->d_flag);
     cudaFree(c->stage);
     if (c->h_ctl) cudaFreeHost(c->h_ctl);
@@ -771,7 +833,7 @@ int nbody_next_block(nbody_ctx *h, int64_t n, const double *t, const double *dt,
     cudaStream_t st = (cudaStream_t)stream;
     SelArgs A;
     fill_select(h, A, n, t, dt, active_idx, /*run_mode=*/0, n);
-    k_select<<<select_grid(c, n), kSelThreads, 0, st>>>(A);
+    k_select<<<select_grid(c, n), kSelThreads, select_smem(c, n), st>>>(A);
     c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
     NB_CUDA(c, cudaMemcpyAsync(c->h_ctl, c->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
@@ -885,7 +947,6 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     // run control
     Ctl *hc = c->h_ctl;
     memset(hc, 0, sizeof(Ctl));
-    hc->min_key = ~0ull;
     hc->t_end = t_end;
     hc->max_blocks = max_blocks;
     NB_CUDA(c, cudaMemcpyAsync(c->d_ctl, hc, sizeof(Ctl), cudaMemcpyHostToDevice, st));
@@ -894,6 +955,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
     fill_select(h, SA, n, t, dt, active_idx, /*run_mode=*/1, max_n_act);
     fill_select(h, SF, n, t, dt, active_idx, /*run_mode=*/2, max_n_act);
     const int sgrid = select_grid(c, n);
+    const size_t ssmem = select_smem(c, n);
     CorrArgs CA;  // the corrector's arguments in control-block mode (shared by K_corr and the fused step)
     {
         CA.idx = active_idx; CA.n_act = 0; CA.t_now = 0.0; CA.eta = eta; CA.dt_min = dt_min; CA.dt_max = dt_max;
@@ -905,7 +967,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         CA.limit_order = c->limit_order; CA.n_limited = &c->d_ctl->limited;
     }
     auto enqueue_step = [&](cudaStream_t s) -> int {  // general step: any block size
-        k_select<<<sgrid, kSelThreads, 0, s>>>(SA);
+        k_select<<<sgrid, kSelThreads, ssmem, s>>>(SA);
         NB_CUDA(c, cudaGetLastError());
         int rc = launch_predict(c, n, 0.0, order, t, m, x, v, a_derivs, c->d_ctl, s);
         if (rc != NBODY_OK) return rc;
@@ -914,7 +976,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         return launch_finish_dyn(c, order, CA, acc, jerk, snap, crackle, pot, s);
     };
     auto enqueue_fused = [&](cudaStream_t s) -> int {  // N1: blocks that fit one i-tile, two launches
-        k_select<<<sgrid, kSelThreads, 0, s>>>(SF);
+        k_select<<<sgrid, kSelThreads, ssmem, s>>>(SF);
         NB_CUDA(c, cudaGetLastError());
         return launch_step_fused(c, order, (float)eps2, active_idx, t, m, x, v, a_derivs, CA, acc, jerk, snap, crackle,
                                  pot, s);

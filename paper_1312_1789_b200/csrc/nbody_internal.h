@@ -76,8 +76,6 @@ __host__ __device__ inline ForceGeo force_geometry(long long n_act, int n_tiles,
 
 // ---- device control block of the device-driven block step (a-1 .. a-4 without host round trips) ---------------
 struct Ctl {
-    unsigned long long min_key;   // order-preserving key of min(t + dt) of the current selection
-    unsigned long long bar;       // monotonic counter of the selection kernel's grid barrier
     double t_next;                // block time of the current block
     double t_end;                 // blocks with t_next > t_end are not executed (stop is set instead)
     long long n_act;              // size of the current block
@@ -90,7 +88,7 @@ struct Ctl {
     long long i_tiles;
     unsigned long long rejected;  // steps refused by the a-posteriori rule (R14) since the counter was last reset
     unsigned long long limited;   // steps taken with a lower-order corrector (R15) since the counter was last reset
-    unsigned int tickets[4];      // last-CTA tickets
+    unsigned int tickets[4];      // last-CTA tickets ([0] fused step, [1] selection)
     unsigned long long hist[40];  // executed blocks by floor(log2 n_act)
 };
 
@@ -110,7 +108,9 @@ struct Ctx {
     size_t partials_bytes = 0;
     int64_t partial_rows = 0;  // S * n_act budget (rows of 13 doubles)
     // selection scratch
-    int *d_counts = nullptr;  // per selection CTA counts
+    int *d_counts = nullptr;  // per selection CTA: particles due at the CTA's own minimum
+    unsigned long long *d_keys = nullptr;  // per selection CTA: that minimum (order-preserving key)
+    int32_t *d_cand = nullptr;  // [cap] their indices (CTA b's slice starts at b * chunk)
     Ctl *d_ctl = nullptr;     // device control block
     Ctl *h_ctl = nullptr;     // pinned host copy (read back after a synchronisation)
     int *d_flag = nullptr;    // validation result
@@ -162,16 +162,11 @@ struct DeviceGuard {
     }
 };
 
-struct SelBar {  // sense-reversing grid barrier of the selection kernel (count + generation)
-    unsigned int count, gen;
-};
-
 }  // namespace nbody
 
 // the opaque handle of include/nbody.h
 struct nbody_ctx {
     nbody::Ctx c;
-    nbody::SelBar *d_bar = nullptr;
     cudaStream_t run_stream = nullptr;  // private stream of nbody_run_blocks (graph capture)
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
 };

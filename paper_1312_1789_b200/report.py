@@ -74,7 +74,7 @@ def sweep(args):
     d_dt = _dev(dt)
     med, best, _ = _time_call(lambda: ctx.next_block(n, st[0], d_dt, act))
     print(json.dumps({"call": "next_block", "config": args.config, "n": n, "us": med * 1e3, "us_best": best * 1e3,
-                      "note": "one kernel + 168-byte D2H + stream synchronise", "algorithmic_GBps": 20 * n / (med * 1e-3) / 1e9}),
+                      "note": "one kernel + D2H of the 424-byte control block + stream synchronise", "algorithmic_GBps": 20 * n / (med * 1e-3) / 1e9}),
           flush=True)
     full = [_dev(d) for d in (D + [np.zeros_like(D[0])] * 8)[:8]]
     sx, sv, sp, s_t, s_dt = st[2].clone(), st[3].clone(), torch.zeros(n, dtype=torch.float64, device="cuda"), st[0].clone(), d_dt.clone()

@@ -65,7 +65,8 @@ def test_null_and_bad_arguments_without_device():
     lib.nbody_workspace_bytes.restype = C.c_int64
     assert lib.nbody_workspace_bytes(C.c_int64(0)) == -1
     w = lib.nbody_workspace_bytes(C.c_int64(2097152))
-    assert 6 * 16 * 2097152 < w < 6 * 16 * 2097152 + (513 << 20)  # j-store + split scratch (<= 512 MB)
+    # j-store + split scratch (<= 512 MB) + selection candidates (4 bytes per particle)
+    assert 6 * 16 * 2097152 < w < 6 * 16 * 2097152 + (513 << 20) + 4 * 2097152
     assert lib.nbody_workspace_bytes(C.c_int64(16)) < 1 << 16     # tiny contexts get a tiny scratch
 
 
