@@ -264,8 +264,8 @@ int nbody_step_host(nbody_ctx *ctx, int64_t n, int order, double eps2, double et
  * nbody_run_blocks -- N2, the device-driven block step ("individual hierarchically block time-steps";
  * PAPER.md:65 eq. (1): the latency term).  Runs whole block steps a-1 .. a-4 (selection, predict, force, correct)
  * back to back WITHOUT the host learning n_act: the selection kernel leaves t_next, n_act and the force geometry in a
- * device control block, the other kernels read them there (persistent grids of fixed size), and the four launches of
- * one block step are replayed as ONE CUDA graph.  The host looks at the control block only every 4 .. 64 block
+ * device control block, the other kernels read them there (persistent grids of fixed size), and the five launches of
+ * one block step (select, predict, force, split reduce, correct) are replayed as ONE CUDA graph.  The host looks at the control block only every 4 .. 64 block
  * steps.  A block is executed iff t_next <= t_end, n_act <= max_n_act and fewer than max_blocks blocks have run; the
  * first block that is not executed ends the run (the state is then exactly the state before that block).
  * Results are bit-identical to the same blocks run through nbody_next_block + nbody_predict + nbody_force +

@@ -973,7 +973,12 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         if (rc != NBODY_OK) return rc;
         rc = launch_force_dyn(c, active_idx, order, (float)eps2, acc, jerk, snap, crackle, pot, s);
         if (rc != NBODY_OK) return rc;
-        return launch_finish_dyn(c, order, CA, acc, jerk, snap, crackle, pot, s);
+        // K_reduce and K_corr as two launches: one fused launch (a warp per particle, the corrector behind its reduce)
+        // measured slower at every size (profiles/r02_latency.md)
+        rc = launch_reduce_dyn(c, order, acc, jerk, snap, crackle, pot, s);
+        if (rc != NBODY_OK) return rc;
+        return launch_correct(c, active_idx, 0, order, 0.0, eta, dt_min, dt_max, kmin, kmax, t, dt, x, v, a_derivs,
+                              pot_state, acc, jerk, snap, crackle, pot, c->d_ctl, s);
     };
     auto enqueue_fused = [&](cudaStream_t s) -> int {  // N1: blocks that fit one i-tile, two launches
         k_select<<<sgrid, kSelThreads, ssmem, s>>>(SF);
@@ -981,7 +986,7 @@ int nbody_run_blocks(nbody_ctx *h, int64_t n, int order, double eps2, double eta
         return launch_step_fused(c, order, (float)eps2, active_idx, t, m, x, v, a_derivs, CA, acc, jerk, snap, crackle,
                                  pot, s);
     };
-    constexpr int kStepLaunches = 4;   // k_select, k_predict, k_force_dyn, k_finish_dyn (K_reduce + K_corr)
+    constexpr int kStepLaunches = 5;   // k_select, k_predict, k_force_dyn, k_reduce_dyn, k_correct
     constexpr int kFusedLaunches = 2;  // k_select, k_step_fused
     const bool fused = c->use_fused != 0;
 

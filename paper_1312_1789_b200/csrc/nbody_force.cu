@@ -24,7 +24,7 @@
 //     through shared memory in fixed order; S > 1 j-splits write fp64 partials [S][NC][n_act] that K_reduce sums
 //     in order.  k_force takes the geometry from the host (grid = i-tiles x S); k_force_dyn is the persistent
 //     form of the same work items (grid = SMs) that reads n_act and the geometry from the device control block
-//     (device-driven block step, nbody_run_blocks); k_finish_dyn is K_reduce + K_corr of that step in one launch.
+//     (device-driven block step, nbody_run_blocks); k_reduce_dyn is K_reduce of that step (S, n_act from the control block).
 #include <math.h>
 
 #include <mutex>
@@ -546,59 +546,12 @@ __global__ void __launch_bounds__(256) k_reduce(const double *partials, int spli
                 (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
-// Device-driven step: K_reduce and K_corr in ONE launch.  S == 1: one thread per active particle runs the corrector.
-// S > 1: one warp per active particle sums its NC outputs over the j-splits -- with exactly the arithmetic of
-// reduce_body for that S (S <= 8: lane c sums component c in sequence; S > 8: per component lane-strided, then the
-// butterfly), so the results are those of k_reduce bit for bit -- and lane 0 then runs the corrector on them.
-template <int ORDER>
-__global__ void __launch_bounds__(256) k_finish_dyn(const Ctl *ctl, const double *partials, const CorrArgs C,
-                                                    double *acc, double *jerk, double *snap, double *crk, double *pot) {
-    if (ctl->stop) return;
-    constexpr int NC = 3 * (ORDER / 2) + 1;
-    const int n_act = (int)ctl->n_act, splits = ctl->splits;
-    const double t_now = ctl->t_next;
-    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nthr = (long long)gridDim.x * blockDim.x;
-    if (splits == 1) {
-        for (long long ia = gtid; ia < n_act; ia += nthr) correct_one<ORDER>(C, ia, t_now);
-        return;
-    }
-    const int lane = threadIdx.x & 31;
-    const long long tot = (long long)NC * n_act;
-    for (long long ia = gtid >> 5; ia < n_act; ia += nthr >> 5) {
-        if (splits <= 8) {
-            if (lane < NC) {
-                const long long o = (long long)lane * n_act + ia;
-                double v[8];
-#pragma unroll
-                for (int k = 0; k < 8; ++k) v[k] = k < splits ? __ldcg(partials + (size_t)k * tot + o) : 0.0;
-                double s = v[0];
-#pragma unroll
-                for (int k = 1; k < 8; ++k)
-                    if (k < splits) s += v[k];
-                reduce_store(s, o, NC, n_act, acc, jerk, snap, crk, pot);
-            }
-        } else {
-            double s[NC];  // all components' loads in flight together (the additions keep reduce_body's order)
-#pragma unroll
-            for (int comp = 0; comp < NC; ++comp) s[comp] = 0.0;
-#pragma unroll 2
-            for (int k = lane; k < splits; k += 32) {
-                double v[NC];
-#pragma unroll
-                for (int comp = 0; comp < NC; ++comp) v[comp] = __ldcg(partials + (size_t)k * tot + (long long)comp * n_act + ia);
-#pragma unroll
-                for (int comp = 0; comp < NC; ++comp) s[comp] += v[comp];
-            }
-#pragma unroll
-            for (int comp = 0; comp < NC; ++comp) {
-#pragma unroll
-                for (int d = 16; d > 0; d >>= 1) s[comp] += __shfl_xor_sync(0xffffffffu, s[comp], d);
-                if (lane == 0) reduce_store(s[comp], (long long)comp * n_act + ia, NC, n_act, acc, jerk, snap, crk, pot);
-            }
-        }
-        __syncwarp();
-        if (lane == 0) correct_one<ORDER>(C, ia, t_now);
-    }
+// K_reduce of the device-driven step: S and n_act from the control block (a stopped run and an unsplit block are no-ops)
+__global__ void __launch_bounds__(256) k_reduce_dyn(const Ctl *ctl, const double *partials, int nc, double *acc,
+                                                    double *jerk, double *snap, double *crk, double *pot) {
+    if (ctl->stop || ctl->splits == 1) return;
+    reduce_body(partials, ctl->splits, nc, (int)ctl->n_act, acc, jerk, snap, crk, pot,
+                (long long)blockIdx.x * blockDim.x + threadIdx.x, (long long)gridDim.x * blockDim.x);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -997,12 +950,9 @@ int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, d
     return NBODY_OK;
 }
 
-int launch_finish_dyn(Ctx *c, int order, const CorrArgs &corr, double *acc, double *jerk, double *snap, double *crackle,
-                      double *pot, cudaStream_t st) {
-    const unsigned grid = 4 * c->sm_count;
-    if (order == 4) k_finish_dyn<4><<<grid, 256, 0, st>>>(c->d_ctl, c->partials, corr, acc, jerk, snap, crackle, pot);
-    else if (order == 6) k_finish_dyn<6><<<grid, 256, 0, st>>>(c->d_ctl, c->partials, corr, acc, jerk, snap, crackle, pot);
-    else k_finish_dyn<8><<<grid, 256, 0, st>>>(c->d_ctl, c->partials, corr, acc, jerk, snap, crackle, pot);
+int launch_reduce_dyn(Ctx *c, int order, double *acc, double *jerk, double *snap, double *crackle, double *pot,
+                      cudaStream_t st) {
+    k_reduce_dyn<<<c->sm_count, 256, 0, st>>>(c->d_ctl, c->partials, 3 * (order / 2) + 1, acc, jerk, snap, crackle, pot);
     NB_CUDA(c, cudaGetLastError());
     return NBODY_OK;
 }

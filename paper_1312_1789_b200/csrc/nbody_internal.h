@@ -183,10 +183,10 @@ int launch_force_dyn(Ctx *c, const int32_t *active_idx, int order, float eps2, d
 int launch_force_static(Ctx *c, const int32_t *active_idx, int64_t n_act, int order, float eps2, double *acc, double *jerk,
                         double *snap, double *crackle, double *pot, cudaStream_t st);
 int force_static_init(Ctx *c);
+// device-driven step: K_reduce with S and n_act from the control block
+int launch_reduce_dyn(Ctx *c, int order, double *acc, double *jerk, double *snap, double *crackle, double *pot,
+                      cudaStream_t st);
 struct CorrArgs;
-// device-driven step: K_reduce + K_corr in one launch (reads n_act, S, t_next from the control block)
-int launch_finish_dyn(Ctx *c, int order, const CorrArgs &corr, double *acc, double *jerk, double *snap, double *crackle,
-                      double *pot, cudaStream_t st);
 // N1: predict + force + reduce + correct of a block that fits one i-tile, in one launch (reads the control block)
 int launch_step_fused(Ctx *c, int order, float eps2, const int32_t *active_idx, const double *t, const double *m,
                       const double *x, const double *v, const double *const a_derivs[8], const CorrArgs &corr,
