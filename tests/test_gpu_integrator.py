@@ -108,6 +108,39 @@ def test_initial_dt_and_next_block_bit_exact(nb, O):
     ctx.close()
 
 
+@pytest.mark.parametrize("n", [1, 31, 1025, 300007, 2600003])
+def test_next_block_chunk_shapes(nb, O, n):
+    """The one-pass selection kernel over its chunk shapes: a single particle, less than a warp, one row per CTA, several
+    rows, and more rows than the shared-memory key cache holds (n > 16 x 1024 x 148).  Blocks: a few scattered particles
+    including the first and the last one, every other particle, a dense stretch inside one chunk, everybody; t_next, n_act
+    and the ascending index list against the oracle, bit for bit."""
+    import torch
+    rng = W.rng_for(3, 77)
+    ctx = nb.Context(n)
+    act = torch.zeros(n, dtype=torch.int32, device="cuda")
+    t = rng.integers(0, 8, n).astype(np.float64) * 2.0**-6
+    dt = 2.0 ** -rng.integers(3, 9, n).astype(np.float64)
+    cases = []
+    few = np.unique(np.concatenate([[0, n - 1], rng.integers(0, n, 13)]))
+    cases.append(few)
+    cases.append(np.arange(0, n, 2))
+    lo = n // 3
+    cases.append(np.arange(lo, min(n, lo + 5000)))
+    cases.append(np.arange(n))
+    for k, due in enumerate(cases):
+        tt, dd = t.copy(), dt.copy()
+        tt += 1.0  # nobody else is due before the chosen block
+        tt[due] = 0.5
+        dd[due] = 2.0**-7
+        tn, oidx = O.next_block(tt, dd)
+        assert tn == 0.5 + 2.0**-7 and np.array_equal(oidx, due.astype(np.int32))
+        act.fill_(-1)
+        gtn, gna = ctx.next_block(n, U.dev(tt), U.dev(dd), act)
+        assert gtn == tn and gna == oidx.shape[0], (n, k, gtn, gna)
+        assert np.array_equal(act[:gna].cpu().numpy(), oidx), (n, k)
+    ctx.close()
+
+
 @pytest.mark.parametrize("order", [4, 6, 8])
 def test_block_integration_vs_oracle(nb, O, order):
     """Scheduler end to end on a small cluster with a central BH: same block sequence (bit-exact membership while
