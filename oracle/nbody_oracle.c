@@ -26,7 +26,9 @@
  * quantisation against exact rational arithmetic (ties and one-ulp near-ties
  * included), the c-8b mean-crackle criterion against its closed form for
  * a(t) = a0 e^(lambda t) (50-digit mpmath), convergence slopes 4/6/8 (table B2),
- * Kepler closure, energy conservation.  Parity unpinned: nothing.
+ * Kepler closure, energy conservation; oracle_nearest (c-17) on a chain with
+ * closed-form neighbours, against an fp64 brute force, on ties and on a
+ * difference only fp64 resolves.  Parity unpinned: nothing.
  */
 #include <math.h>
 #include <stddef.h>
@@ -235,6 +237,42 @@ void oracle_force_abs(int64_t n, const double *m,
 }
 
 /* Euclidean norm, fixed order ((x^2 + y^2) + z^2) then IEEE sqrt. */
+/* ------------------------------------------------------------------------
+ * c-17 (this build's reading R16 of SURVEY 8(f) N4 "nearest-neighbour output";
+ * not in PAPER.md, which names the Ahmad-Cohen neighbour scheme of its second
+ * code only): for every active particle the index of the nearest
+ * OTHER particle (excluded by index, as in c-1) at the predicted positions, and
+ * the squared distance to it.  The distance decides an integer (the argmin), so
+ * its precision is fixed and is the force kernel's (c-12): each component of
+ * the difference is formed in fp64 and rounded to fp32, and
+ *     r2 = fma(dz, dz, fma(dy, dy, dx * dx))      in fp32, in this order;
+ * ties go to the lowest index.  n == 1: index -1, r2 = +inf.
+ * nn_r2 holds the fp32 value (as a double).
+ * ------------------------------------------------------------------------ */
+void oracle_nearest(int64_t n, const double *xp, const int32_t *active_idx, int64_t n_act,
+                    int32_t *nn_idx, double *nn_r2)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t ia = 0; ia < n_act; ++ia) {
+        const int64_t i = active_idx[ia];
+        float best = INFINITY;
+        int32_t who = -1;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            const float dx = (float)(xp[3 * j + 0] - xp[3 * i + 0]);
+            const float dy = (float)(xp[3 * j + 1] - xp[3 * i + 1]);
+            const float dz = (float)(xp[3 * j + 2] - xp[3 * i + 2]);
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (r2 < best) {
+                best = r2;
+                who = (int32_t)j;
+            }
+        }
+        nn_idx[ia] = who;
+        nn_r2[ia] = (double)best;
+    }
+}
+
 static double nrm3(const double *a)
 {
     return sqrt((a[0] * a[0] + a[1] * a[1]) + a[2] * a[2]);

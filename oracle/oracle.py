@@ -29,6 +29,8 @@ def lib():
         L.oracle_force_abs.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, _dp, _ip, C.c_int64, C.c_int, C.c_double,
                                        _dp, _dp, _dp, _dp]
         L.oracle_force_abs.restype = None
+        L.oracle_nearest.argtypes = [C.c_int64, _dp, _ip, C.c_int64, _ip, _dp]
+        L.oracle_nearest.restype = None
         L.oracle_new_dt.argtypes = [C.c_int, C.POINTER(_dp), C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
         L.oracle_new_dt.restype = C.c_double
         L.oracle_initial_dt.argtypes = [C.c_int64, _dp, _dp, C.c_double, C.c_double, C.c_double, _dp]
@@ -115,6 +117,16 @@ def force_abs(m, xp, vp, ap, jp, active_idx, order, eps2):
     lib().oracle_force_abs(n, _p(m), _p(xp), _p(vp), _p(ap), _p(jp), idx.ctypes.data_as(_ip), na, order, float(eps2),
                            _p(a), _p(j), _p(s), _p(c))
     return a, j, s, c
+
+
+def nearest(xp, active_idx):
+    """c-17: (index, squared distance in the force kernel's fp32) of the nearest other particle of each active one."""
+    xp = _d(xp)
+    idx = np.ascontiguousarray(active_idx, dtype=np.int32)
+    who = np.empty(idx.shape[0], dtype=np.int32)
+    r2 = np.empty(idx.shape[0])
+    lib().oracle_nearest(xp.shape[0], _p(xp), idx.ctypes.data_as(_ip), idx.shape[0], who.ctypes.data_as(_ip), _p(r2))
+    return who, r2
 
 
 def new_dt(order, derivs, t1, dt_old, eta, dt_min, dt_max):
