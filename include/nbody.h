@@ -224,6 +224,20 @@ int nbody_initial_dt(nbody_ctx *ctx, int64_t n, const double *acc, const double 
 int nbody_next_block(nbody_ctx *ctx, int64_t n, const double *t, const double *dt,
                      int32_t *active_idx, double *t_next_host, int64_t *n_act_host, void *stream);
 
+/* ------------------------------------------------------------------------------------------------------------
+ * nbody_nearest -- SURVEY 8(f) N4 "nearest-neighbour output" (reading R16, oracle c-17; not in PAPER.md, which only
+ * names the neighbour scheme of its second code).  For each active i (index into the j-store of the last
+ * nbody_predict) the nearest OTHER particle (excluded by index) at the predicted positions:
+ *     d = fl32(x_j - x_i), each component formed in fp64 (the force kernel's differences, R10);
+ *     r2 = fma(dz, dz, fma(dy, dy, dx * dx)) in fp32;  the smallest r2 wins, ties go to the lowest j.
+ *   nn_idx: device int32 [n_act] (-1 when n == 1); nn_r2: device fp64 [n_act] holding the fp32 value (+inf when
+ *   n == 1), both in ACTIVE-LIST order.  Bit-exact against the oracle; independent of the launch geometry.
+ *   Uses the ctx's split scratch (as nbody_force does): order it with the other calls on this ctx by the stream.
+ * Errors: EINVAL (n_act < 0, n_act > n, NULL or misaligned pointer, validation failure), ESTATE (no predict yet),
+ * ENOMEM (n_act * 8 bytes beyond the split scratch: cannot happen below 67 M particles).  n_act == 0 is a no-op.
+ * ---------------------------------------------------------------------------------------------------------- */
+int nbody_nearest(nbody_ctx *ctx, const int32_t *active_idx, int64_t n_act, int32_t *nn_idx, double *nn_r2, void *stream);
+
 /* count_host[0] = steps refused by the "step_reject_ratio" rule, count_host[1] = steps taken with a lower-order corrector
  * ("corrector_order_limit"), since the counters were last reset (nbody_run_blocks resets them at the start of every run);
  * reset != 0 clears them.  count_host is a HOST array of 2; synchronises `stream`. */

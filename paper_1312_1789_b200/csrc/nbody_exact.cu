@@ -94,6 +94,68 @@ __global__ void k_unpack(const uint4 *q0, const uint4 *q1, const uint4 *q2, cons
     }
 }
 
+// ---- nearest-neighbour output (reading R16 = oracle c-17) -----------------------------------------
+// For each active i the nearest other particle of the j-store: d = fl32(x_j - x_i) formed in fp64 (the force kernel's
+// differences), r2 = fma(dz, dz, fma(dy, dy, dx * dx)) in fp32, ties to the lowest index.  One thread per active
+// particle, j-tiles of kNnTile staged in shared memory, S j-splits; the splits meet in an atomicMin on the 64-bit key
+// (bits of r2) << 32 | j -- r2 >= 0, so the order of the keys is the order of (r2, j) and the result does not depend
+// on S or on the order in which the splits arrive.
+constexpr int kNnTile = 256;
+
+__global__ void __launch_bounds__(kNnTile) k_nearest(const uint4 *q0, const uint4 *q1, long long n,
+                                                      const int32_t *active_idx, int n_act, int n_tiles, int splits,
+                                                      unsigned long long *keys) {
+    __shared__ uint4 s0[kNnTile], s1[kNnTile];
+    const int tid = threadIdx.x;
+    const int ia = blockIdx.x * kNnTile + tid;
+    const bool live = ia < n_act;
+    const int i = live ? active_idx[ia] : 0;
+    double xi = 0.0, yi = 0.0, zi = 0.0;
+    if (live) {
+        const uint4 a = q0[i], b = q1[i];
+        xi = __longlong_as_double(((long long)a.y << 32) | a.x);
+        yi = __longlong_as_double(((long long)a.w << 32) | a.z);
+        zi = __longlong_as_double(((long long)b.y << 32) | b.x);
+    }
+    const int per = (n_tiles + splits - 1) / splits;
+    const int tile_lo = blockIdx.y * per, tile_hi = tile_lo + per < n_tiles ? tile_lo + per : n_tiles;
+    unsigned long long best = ~0ull;
+    for (int tile = tile_lo; tile < tile_hi; ++tile) {
+        const long long j0 = (long long)tile * kNnTile;
+        __syncthreads();
+        if (j0 + tid < n) {
+            s0[tid] = q0[j0 + tid];
+            s1[tid] = q1[j0 + tid];
+        }
+        __syncthreads();
+        const int cnt = n - j0 < kNnTile ? (int)(n - j0) : kNnTile;
+#pragma unroll 4
+        for (int jj = 0; jj < cnt; ++jj) {
+            const uint4 a = s0[jj], b = s1[jj];
+            const float dx = __double2float_rn(__dsub_rn(__longlong_as_double(((long long)a.y << 32) | a.x), xi));
+            const float dy = __double2float_rn(__dsub_rn(__longlong_as_double(((long long)a.w << 32) | a.z), yi));
+            const float dz = __double2float_rn(__dsub_rn(__longlong_as_double(((long long)b.y << 32) | b.x), zi));
+            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const unsigned long long key = ((unsigned long long)__float_as_uint(r2) << 32) | (unsigned)(j0 + jj);
+            if (j0 + jj != i && r2 == r2 && key < best) best = key;  // ascending j: a tie keeps the earlier one
+        }
+    }
+    if (live && best != ~0ull) atomicMin(keys + ia, best);
+}
+
+__global__ void k_nearest_out(const unsigned long long *keys, int n_act, int32_t *nn_idx, double *nn_r2) {
+    const int ia = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ia >= n_act) return;
+    const unsigned long long k = keys[ia];
+    if (k == ~0ull) {  // no other particle
+        nn_idx[ia] = -1;
+        nn_r2[ia] = __longlong_as_double(0x7ff0000000000000ll);
+    } else {
+        nn_idx[ia] = (int32_t)(k & 0xffffffffull);
+        nn_r2[ia] = (double)__uint_as_float((unsigned)(k >> 32));
+    }
+}
+
 }  // namespace
 
 // K_pred's particle arithmetic and the whole of K_corr (k_correct, correct_one) live in nbody_exact.cuh.
@@ -855,6 +917,40 @@ int nbody_get_predicted(nbody_ctx *h, double *xp, float *vp, float *ap, float *j
         q, q + c->cap_pad, q + 2 * c->cap_pad, q + 3 * c->cap_pad, c->n, c->pred_order, xp, vp, ap, jp, m32);
     c->launches += 1;
     NB_CUDA(c, cudaGetLastError());
+    return NBODY_OK;
+}
+
+int nbody_nearest(nbody_ctx *h, const int32_t *active_idx, int64_t n_act, int32_t *nn_idx, double *nn_r2, void *stream) {
+    if (!h || n_act < 0) return NBODY_EINVAL;
+    Ctx *c = &h->c;
+    if (c->n < 0) return NBODY_ESTATE;
+    if (n_act > c->n) return NBODY_EINVAL;
+    if (n_act == 0) return NBODY_OK;
+    if (!active_idx || !nn_idx || !nn_r2) return NBODY_EINVAL;
+    NB_ALIGN8(nn_r2);
+    if (misaligned(active_idx, 4) || misaligned(nn_idx, 4)) return NBODY_EINVAL;
+    if ((size_t)n_act * sizeof(unsigned long long) > c->partials_bytes) return NBODY_ENOMEM;  // keys live in the split scratch
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->validate) {
+        const int rc = validate_active(c, active_idx, n_act, c->n, nullptr, nullptr, 0.0, st);
+        if (rc != NBODY_OK) return rc;
+    }
+    unsigned long long *keys = reinterpret_cast<unsigned long long *>(c->partials);
+    NB_CUDA(c, cudaMemsetAsync(keys, 0xff, (size_t)n_act * sizeof(unsigned long long), st));
+    const int n_tiles = (int)((c->n + kNnTile - 1) / kNnTile);
+    const long long i_tiles = (n_act + kNnTile - 1) / kNnTile;
+    long long S = (4LL * c->sm_count + i_tiles - 1) / i_tiles;  // about four CTAs per SM in flight
+    if (S > n_tiles) S = n_tiles;
+    if (S > 65535) S = 65535;
+    if (S < 1) S = 1;
+    const uint4 *q = c->jstore;
+    k_nearest<<<dim3((unsigned)i_tiles, (unsigned)S), kNnTile, 0, st>>>(q, q + c->cap_pad, c->n, active_idx, (int)n_act,
+                                                                        n_tiles, (int)S, keys);
+    NB_CUDA(c, cudaGetLastError());
+    k_nearest_out<<<(unsigned)((n_act + 255) / 256), 256, 0, st>>>(keys, (int)n_act, nn_idx, nn_r2);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 2;
     return NBODY_OK;
 }
 

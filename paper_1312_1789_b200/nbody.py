@@ -50,6 +50,7 @@ SIGNATURES = {
     "nbody_initial_dt": (C.c_int, [_vp, _i64, _vp, _vp, _dbl, _dbl, _dbl, _vp, _vp]),
     "nbody_next_block": (C.c_int, [_vp, _i64, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_i64), _vp]),
     "nbody_get_predicted": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nbody_nearest": (C.c_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
     "nbody_rejected_steps": (C.c_int, [_vp, C.c_int, C.POINTER(_i64), _vp]),
     "nbody_run_blocks": (C.c_int, [_vp, _i64, C.c_int, _dbl, _dbl, _dbl, _dbl, _dbl, _i64, _i64, _vp, _vp, _vp, _vp, _vp,
                                    C.POINTER(_vp), _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.POINTER(RunResult), _vp]),
@@ -168,6 +169,12 @@ class Context:
                                        float(dt_min), float(dt_max), _ptr(t), _ptr(dt), _ptr(x), _ptr(v),
                                        _ptr_array(a_derivs, 8), _ptr(pot_state), _ptr(acc), _ptr(jerk), _ptr(snap),
                                        _ptr(crackle), _ptr(pot), _stream(stream)), "nbody_correct")
+
+    def nearest(self, active_idx, n_act, nn_idx, nn_r2, stream=None):
+        """N4 neighbour output: index (int32) and squared distance (fp64 holding the fp32 value) of the nearest other
+        particle of each active one, at the positions of the last predict."""
+        self._check(_lib.nbody_nearest(self._h, _ptr(active_idx), int(n_act), _ptr(nn_idx), _ptr(nn_r2), _stream(stream)),
+                    "nbody_nearest")
 
     def initial_dt(self, n, acc, jerk, eta_s, dt_min, dt_max, dt, stream=None):
         self._check(_lib.nbody_initial_dt(self._h, int(n), _ptr(acc), _ptr(jerk), float(eta_s), float(dt_min),
