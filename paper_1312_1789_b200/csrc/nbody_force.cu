@@ -491,7 +491,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_force_dyn(const ForceArgs A) {
             case 2: force_item<ORDER, 2, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             case 4: force_item<ORDER, 4, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             case 8: force_item<ORDER, 8, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 16: force_item<ORDER, 16, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             case 32: force_item<ORDER, 32, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 64: force_item<ORDER, 64, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             default: force_item<ORDER, 128, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
         }
         __syncthreads();  // the epilogue has read the accumulators before the next item clears them
@@ -792,7 +794,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_step_fused(const FusedArgs A) {
             case 2: fused_item<ORDER, 2>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             case 4: fused_item<ORDER, 4>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             case 8: fused_item<ORDER, 8>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 16: fused_item<ORDER, 16>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             case 32: fused_item<ORDER, 32>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 64: fused_item<ORDER, 64>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             default: fused_item<ORDER, 128>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
         }
         __syncthreads();
@@ -826,7 +830,9 @@ force_fn pick(int jl) {
         case 2: return k_force<ORDER, 2, DIFF>;
         case 4: return k_force<ORDER, 4, DIFF>;
         case 8: return k_force<ORDER, 8, DIFF>;
+        case 16: return k_force<ORDER, 16, DIFF>;
         case 32: return k_force<ORDER, 32, DIFF>;
+        case 64: return k_force<ORDER, 64, DIFF>;
         default: return k_force<ORDER, 128, DIFF>;
     }
 }

@@ -110,8 +110,8 @@ def test_force_geometry_rule_matches_round1_table():
     prog = """#include <stdio.h>
 #define __host__
 #define __device__
-constexpr int kThreads = 512, kNumLanes = 6;
-inline int lane_variant(int k) { return k == 0 ? 1 : k == 1 ? 2 : k == 2 ? 4 : k == 3 ? 8 : k == 4 ? 32 : 128; }
+constexpr int kThreads = 512, kNumLanes = 8;
+inline int lane_variant(int k) { return 1 << k; }
 %s
 int main() {
     const long long cases[][2] = {{1, 256}, {16, 256}, {256, 256}, {4096, 256}, {65536, 256}, {1, 1024}, {64, 1024},
@@ -128,12 +128,12 @@ int main() {
         out = subprocess.run([os.path.join(d, "g")], capture_output=True, text=True).stdout.split("\n")
     got = {(int(l.split()[0]), int(l.split()[1])): tuple(int(v) for v in l.split()[2:]) for l in out if l.strip()}
     assert got[(1, 256)] == (128, 128, 1)
-    assert got[(16, 256)] == (32, 128, 1)
+    assert got[(16, 256)] == (64, 128, 1)
     assert got[(256, 256)] == (4, 128, 1)
     assert got[(4096, 256)] == (1, 37, 4)
     assert got[(65536, 256)] == (1, 9, 64)
     assert got[(1, 1024)] == (128, 147, 1)
-    assert got[(64, 1024)] == (8, 147, 1)
+    assert got[(64, 1024)] == (16, 147, 1)
     assert got[(1024, 1024)] == (1, 147, 1)
     assert got[(262144, 1024)] == (1, 4, 256)
     assert got[(1048576, 4096)] == (1, 1, 1024)
