@@ -77,7 +77,7 @@ int nbody_last_cuda_error(const nbody_ctx *ctx);
  *                 criterion of R8, which fp32 force noise collapses for p >= 6 (R8b): fp64 forces only.
  *   "force_split" 0 = automatic j-split, S >= 1 = force exactly S j-splits (tests: split independence); a forced S
  *                 with S * n_act beyond the split scratch makes nbody_force return NBODY_EINVAL
- *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 4, ..., 128)
+ *   "force_lanes" 0 = automatic, else force the j-lanes-per-CTA variant (1, 2, 4, ..., 256)
  *   "geometry_n_act" 0 = the call's n_act decides the j-lane variant and the j-split [default]; G > 0 = decide as if the
  *                 call had G active particles (G >= n_act).  An i-sharded rank passes its slice of the active list and
  *                 G = the size of the whole block: every particle is then summed in exactly the order of the unsharded

@@ -740,7 +740,7 @@ int nbody_set_option(nbody_ctx *h, const char *key, int64_t value) {
         return NBODY_OK;
     }
     if (!strcmp(key, "force_lanes")) {
-        if (value != 0 && !(value >= 1 && value <= 128 && (value & (value - 1)) == 0)) return NBODY_EINVAL;
+        if (value != 0 && !(value >= 1 && value <= 256 && (value & (value - 1)) == 0)) return NBODY_EINVAL;
         c->force_lanes = (int)value;
         return NBODY_OK;
     }

@@ -20,7 +20,7 @@
 //     executed by warps whose i-indices fall inside the current j-tile or whose tile holds pads (warp-uniform
 //     branch), so the main loop is mask-free;
 //   - a work item is (i-tile, j-split): IT = kThreads/JL i-lanes x JL j-lanes (2 IT i-particles): JL = 1 for big
-//     blocks (every lane reads the same j: smem broadcast), JL up to 128 for tiny blocks; the j-lanes are reduced
+//     blocks (every lane reads the same j: smem broadcast), JL up to 256 for tiny blocks; the j-lanes are reduced
 //     through shared memory in fixed order; S > 1 j-splits write fp64 partials [S][NC][n_act] that K_reduce sums
 //     in order.  k_force takes the geometry from the host (grid = i-tiles x S); k_force_dyn is the persistent
 //     form of the same work items (grid = SMs) that reads n_act and the geometry from the device control block
@@ -311,6 +311,43 @@ __device__ __forceinline__ void tile_compute(const IPair<ORDER, DIFF> &I, const 
 // One work item = (i-tile, j-split) of a force call.  `tile_run` counts the j-tiles this CTA has pushed through the
 // ring since its mbarriers were initialised (stage and phase of tile g are g % STAGES and (g / STAGES) & 1), so a
 // persistent CTA runs item after item on the same barriers.
+// Epilogue of a work item with JL >= 128 j-lanes (few outputs, long sums; shared by force_item and fused_item, so every
+// path sums in the same order): the fp64 accumulators of the JL j-lanes of each output are summed in a FIXED order by
+// T = 4 (JL = 128) or 8 (JL = 256) adjacent threads -- thread t sums lanes l = t, t + T, ... in sequence, then a butterfly
+// over the T threads -- pot is negated, and the result goes to the output arrays (S == 1) or to this split's row of the
+// partials (S > 1).  (JL <= 64: one thread per output, lanes l = 0 .. JL-1 in sequence, written out at the call sites.)
+template <int JL, int NC>
+__device__ __forceinline__ void lane_sum_store(const ForceArgs &A, const double *acc_sm, int i_tile, int n_act,
+                                               int splits, int split) {
+    constexpr int IT = kThreads / JL;
+    constexpr int NOUT = 2 * IT * NC;
+    constexpr int T = JL >= 256 ? 8 : JL >= 128 ? 4 : 1;
+    const int tid = threadIdx.x;
+    for (int base = 0; base < NOUT * T; base += kThreads) {  // uniform trip count: the shuffles below see full warps
+        const int q = base + tid;
+        const int o = q / T, t = q % T;
+        const int comp = o / (2 * IT), rem = o % (2 * IT);
+        const int r = rem / IT, i_l = rem % IT;
+        double sum = 0.0;
+        if (o < NOUT) {
+#pragma unroll 8
+            for (int l = t; l < JL; l += T) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
+        }
+#pragma unroll
+        for (int d = T / 2; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+        const int slot = i_tile * (2 * IT) + r * IT + i_l;
+        if (o < NOUT && t == 0 && slot < n_act) {
+            if (comp == NC - 1) sum = -sum;
+            if (splits == 1) {
+                if (comp == NC - 1) A.out[4][slot] = sum;
+                else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
+            } else {
+                A.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+            }
+        }
+    }
+}
+
 template <int ORDER, int JL, int DIFF>
 __device__ __forceinline__ void force_item(const ForceArgs &A, const int n_act, const int splits, const int i_tile,
                                            const int split, unsigned char *smem_raw, unsigned &tile_run) {
@@ -430,20 +467,24 @@ __device__ __forceinline__ void force_item(const ForceArgs &A, const int n_act, 
     __syncthreads();
 
     // ---- epilogue: fixed-order sum over the JL j-lanes, pot = - Sum m/r ----
-    for (int o = tid; o < 2 * IT * NC; o += kThreads) {
-        const int comp = o / (2 * IT), rem = o % (2 * IT);
-        const int r = rem / IT, i_l = rem % IT;
-        double sum = 0.0;
+    if constexpr (JL >= 128) {
+        lane_sum_store<JL, NC>(A, acc_sm, i_tile, n_act, splits, split);
+    } else {  // one thread per output, lanes in sequence (kept as written: the big-block kernels are tuned around it)
+        for (int o = tid; o < 2 * IT * NC; o += kThreads) {
+            const int comp = o / (2 * IT), rem = o % (2 * IT);
+            const int r = rem / IT, i_l = rem % IT;
+            double sum = 0.0;
 #pragma unroll 8
-        for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
-        const int slot = i_tile * (2 * IT) + r * IT + i_l;
-        if (slot < n_act) {
-            if (comp == NC - 1) sum = -sum;
-            if (splits == 1) {
-                if (comp == NC - 1) A.out[4][slot] = sum;
-                else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
-            } else {
-                A.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+            for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
+            const int slot = i_tile * (2 * IT) + r * IT + i_l;
+            if (slot < n_act) {
+                if (comp == NC - 1) sum = -sum;
+                if (splits == 1) {
+                    if (comp == NC - 1) A.out[4][slot] = sum;
+                    else A.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
+                } else {
+                    A.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+                }
             }
         }
     }
@@ -494,7 +535,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_force_dyn(const ForceArgs A) {
             case 16: force_item<ORDER, 16, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             case 32: force_item<ORDER, 32, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
             case 64: force_item<ORDER, 64, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
-            default: force_item<ORDER, 128, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            case 128: force_item<ORDER, 128, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
+            default: force_item<ORDER, 256, 0>(A, n_act, splits, i_tile, split, smem_raw, tile_run); break;
         }
         __syncthreads();  // the epilogue has read the accumulators before the next item clears them
     }
@@ -747,21 +789,25 @@ __device__ __forceinline__ void fused_item(const FusedArgs &A, const int n_act, 
     flush(pa, acc_mine);
     __syncthreads();
 
-    // ---- epilogue: fixed-order sum over the JL j-lanes, pot = - Sum m/r (as force_item, i-tile 0) ----
-    for (int o = tid; o < 2 * IT * NC; o += kThreads) {
-        const int comp = o / (2 * IT), rem = o % (2 * IT);
-        const int r = rem / IT, i_l = rem % IT;
-        double sum = 0.0;
+    // ---- epilogue: force_item's, for i-tile 0 ----
+    if constexpr (JL >= 128) {
+        lane_sum_store<JL, NC>(F, acc_sm, 0, n_act, splits, split);
+    } else {
+        for (int o = tid; o < 2 * IT * NC; o += kThreads) {
+            const int comp = o / (2 * IT), rem = o % (2 * IT);
+            const int r = rem / IT, i_l = rem % IT;
+            double sum = 0.0;
 #pragma unroll 8
-        for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
-        const int slot = r * IT + i_l;
-        if (slot < n_act) {
-            if (comp == NC - 1) sum = -sum;
-            if (splits == 1) {
-                if (comp == NC - 1) F.out[4][slot] = sum;
-                else F.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
-            } else {
-                F.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+            for (int l = 0; l < JL; ++l) sum += acc_sm[(2 * comp + r) * kThreads + l * IT + i_l];
+            const int slot = r * IT + i_l;
+            if (slot < n_act) {
+                if (comp == NC - 1) sum = -sum;
+                if (splits == 1) {
+                    if (comp == NC - 1) F.out[4][slot] = sum;
+                    else F.out[comp / 3][(size_t)slot * 3 + comp % 3] = sum;
+                } else {
+                    F.partials[((size_t)split * NC + comp) * n_act + slot] = sum;
+                }
             }
         }
     }
@@ -797,7 +843,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_step_fused(const FusedArgs A) {
             case 16: fused_item<ORDER, 16>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             case 32: fused_item<ORDER, 32>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
             case 64: fused_item<ORDER, 64>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
-            default: fused_item<ORDER, 128>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            case 128: fused_item<ORDER, 128>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
+            default: fused_item<ORDER, 256>(A, n_act, splits, w, t_now, smem_raw, tile_run); break;
         }
         __syncthreads();
     }
@@ -833,7 +880,8 @@ force_fn pick(int jl) {
         case 16: return k_force<ORDER, 16, DIFF>;
         case 32: return k_force<ORDER, 32, DIFF>;
         case 64: return k_force<ORDER, 64, DIFF>;
-        default: return k_force<ORDER, 128, DIFF>;
+        case 128: return k_force<ORDER, 128, DIFF>;
+        default: return k_force<ORDER, 256, DIFF>;
     }
 }
 

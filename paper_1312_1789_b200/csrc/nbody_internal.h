@@ -20,10 +20,10 @@ constexpr int kPlanes = 6;
 constexpr int kTileJ = 256;    // j-particles per TMA stage (and the padding granule of the j-store)
 constexpr int kThreads = 512;  // threads per force CTA (one CTA per SM)
 constexpr double kPadPos = 1.0e6;
-constexpr int kNumLanes = 8;   // j-lane variants of the force kernel: a CTA is (kThreads / JL) i-lanes x JL j-lanes
+constexpr int kNumLanes = 9;   // j-lane variants of the force kernel: a CTA is (kThreads / JL) i-lanes x JL j-lanes
 
 __host__ __device__ inline int lane_variant(int k) {
-    return 1 << k;  // 1, 2, 4, 8, 16, 32, 64, 128
+    return 1 << k;  // 1, 2, 4, ..., 256 (256 = kTileJ: one j per thread and tile)
 }
 
 // ---- launch geometry of K_force (a-3), shared by the host launcher and the device-driven block step --------

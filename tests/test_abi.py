@@ -110,7 +110,7 @@ def test_force_geometry_rule_matches_round1_table():
     prog = """#include <stdio.h>
 #define __host__
 #define __device__
-constexpr int kThreads = 512, kNumLanes = 8;
+constexpr int kThreads = 512, kNumLanes = 9;
 inline int lane_variant(int k) { return 1 << k; }
 %s
 int main() {
@@ -127,12 +127,12 @@ int main() {
         subprocess.check_call(["g++", "-std=c++17", "-O1", "-o", os.path.join(d, "g"), os.path.join(d, "g.cpp")])
         out = subprocess.run([os.path.join(d, "g")], capture_output=True, text=True).stdout.split("\n")
     got = {(int(l.split()[0]), int(l.split()[1])): tuple(int(v) for v in l.split()[2:]) for l in out if l.strip()}
-    assert got[(1, 256)] == (128, 128, 1)
+    assert got[(1, 256)] == (256, 128, 1)
     assert got[(16, 256)] == (64, 128, 1)
     assert got[(256, 256)] == (4, 128, 1)
     assert got[(4096, 256)] == (1, 37, 4)
     assert got[(65536, 256)] == (1, 9, 64)
-    assert got[(1, 1024)] == (128, 147, 1)
+    assert got[(1, 1024)] == (256, 147, 1)
     assert got[(64, 1024)] == (16, 147, 1)
     assert got[(1024, 1024)] == (1, 147, 1)
     assert got[(262144, 1024)] == (1, 4, 256)

@@ -113,7 +113,7 @@ def test_force_split_and_lane_independence(nb, O):
     for a, b in zip(base, again):
         if a is not None:
             assert np.array_equal(a, b)
-    for split, lanes in ((1, 0), (2, 0), (7, 0), (12, 0), (0, 1), (0, 2), (0, 4), (0, 8), (0, 16), (0, 32), (0, 64), (0, 128), (3, 128), (5, 16), (2, 64)):
+    for split, lanes in ((1, 0), (2, 0), (7, 0), (12, 0), (0, 1), (0, 2), (0, 4), (0, 8), (0, 16), (0, 32), (0, 64), (0, 128), (0, 256), (3, 128), (5, 16), (2, 64), (4, 256)):
         ctx.set_option("force_split", split)
         ctx.set_option("force_lanes", lanes)
         got = U.gpu_force(ctx, n, order, c["eps2"], 0.0, t, c["m"], c["x"], c["v"], D, idx)
