@@ -14,9 +14,9 @@
  *   - Unless a parameter is marked HOST, every array pointer is a DEVICE pointer into caller-owned memory,
  *     fp64, contiguous, 8-byte aligned (int32 arrays 4-byte aligned; anything else is NBODY_EINVAL); 3-vectors are
  *     row-major [n][3].  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *     nbody_predict / nbody_force / nbody_correct / nbody_initial_dt / nbody_get_predicted / nbody_pack_rows /
- *     nbody_unpack_rows only enqueue work and return: they never synchronise and never allocate (all scratch is sized
- *     in nbody_create).  Calls that return a value to the host say so (nbody_next_block, nbody_run_blocks, *_host);
+ *     nbody_predict / nbody_force / nbody_force_static / nbody_nearest / nbody_correct / nbody_initial_dt /
+ *     nbody_get_predicted / nbody_pack_rows / nbody_unpack_rows only enqueue work and return: they never synchronise
+ *     and never allocate (all scratch is sized in nbody_create).  Calls that return a value to the host say so (nbody_next_block, nbody_run_blocks, *_host);
  *     with the "validate" option on, nbody_force and nbody_correct also synchronise (debug mode).
  *   - The ctx owns scratch only (packed j-store, split partials, control block, staging for the *_host calls).  It
  *     never frees or keeps caller memory.  A ctx is bound to the device given at creation: every call switches to that
@@ -53,11 +53,12 @@ const char *nbody_strerror(int code);
 /* Create a context for up to n_capacity particles on CUDA device `device`.  Allocates, with cudaMalloc, the packed
  * j-store (6 planes x 16 B x n_capacity rounded up to the 256-particle j-tile; 4 of them in use unless diff_mode is
  * 1), the j-split scratch (rows of 13 doubles: max(4 SMs x 1024, 4 n_capacity) rows, at most 512 MB; the split
- * heuristic never asks for more, so nbody_force never allocates) and small control blocks.  *out is set only on
+ * heuristic never asks for more, so nbody_force never allocates), the selection's candidate list (4 B x n_capacity)
+ * and small control blocks.  *out is set only on
  * success.  Synchronises the device; the caller's current device is left unchanged. */
 int nbody_create(nbody_ctx **out, int64_t n_capacity, int device);
 
-/* Device bytes nbody_create(n_capacity) allocates on a 148-SM part (j-store + split scratch + control blocks);
+/* Device bytes nbody_create(n_capacity) allocates on a 148-SM part (j-store + split scratch + selection candidates + control blocks);
  * -1 for an invalid capacity.  HOST arithmetic only. */
 int64_t nbody_workspace_bytes(int64_t n_capacity);
 
