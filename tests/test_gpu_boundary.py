@@ -49,6 +49,15 @@ def test_alignment_and_eps2_flush_are_rejected():
     assert e.value.code == nb.EINVAL
     with pytest.raises(nb.NBodyError):
         ctx.set_option("geometry_n_act", 101)
+    for bad in (3, 512, -1):  # the j-lane variants are the powers of two up to 256
+        with pytest.raises(nb.NBodyError) as e:
+            ctx.set_option("force_lanes", bad)
+        assert e.value.code == nb.EINVAL
+    for ok in (256, 16, 0):
+        ctx.set_option("force_lanes", ok)
+    with pytest.raises(nb.NBodyError) as e:
+        ctx.set_option("no_such_option", 1)
+    assert e.value.code == nb.EINVAL
     ctx.set_option("geometry_n_act", 5)
     with pytest.raises(nb.NBodyError) as e:
         ctx.force(idx, 10, 4, 1e-4, z, z, None, None, z1)  # n_act above the declared block size
